@@ -1,0 +1,118 @@
+/*
+ * ptfock.h -- C ABI of the B200-native plane-wave Fock exchange library (libptfock.so).
+ *
+ * The operation (Sec. 2, Eq. (3); Sec. 3.2, Alg. 2 lines 6-10):
+ *
+ *     (V_X[Phi] psi_j)(r) = - alpha * sum_i phi_i(r) * IFFT[ v(G) * FFT( conj(phi_i) psi_j ) ](r)
+ *
+ * on a periodic cell with a regular real-space grid n = (n0, n1, n2), N = n0 n1 n2 points.
+ * Forward DFT exp(-i), unnormalised; inverse exp(+i) with 1/N (any consistent pair gives the same
+ * result).  v(G) is evaluated on every grid frequency m_d in [-n_d/2, n_d/2):
+ *     PTFOCK_KERNEL_COULOMB : 4 pi / |G|^2,                              v(0) = 0
+ *     PTFOCK_KERNEL_HSE     : 4 pi / |G|^2 * (1 - exp(-|G|^2/(4 omega^2))), v(0) = pi / omega^2
+ * ("kernel for the (possibly screened) electron-electron interaction"; the formulas are
+ * BASELINE.json north_star's; the paper prints none -- DESIGN.md readings Q1-Q3).
+ *
+ * Array layout: C order [orbital][x0][x1][x2], x2 contiguous, interleaved (re, im) IEEE fp64,
+ * i.e. one grid = 16 N bytes, orbital k starts at byte 16 N k.  All orbital pointers must be
+ * 16-byte aligned.  Unless a function says HOST, pointers are DEVICE pointers on the plan's device.
+ *
+ * Everything runs in hand-written sm_100a kernels; there is no CPU fallback: on a machine without
+ * such a device ptfock_create returns PTFOCK_ERR_UNSUPPORTED_DEVICE (or PTFOCK_ERR_CUDA).
+ *
+ * Error behaviour: every function returns 0 (PTFOCK_OK) or a negative code below; nothing throws
+ * or aborts across the ABI.  A plan is not thread-safe; distinct plans are independent.
+ */
+#ifndef PTFOCK_H
+#define PTFOCK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ptfock_plan ptfock_plan; /* opaque, owned by the library */
+
+enum {
+    PTFOCK_KERNEL_COULOMB = 0,
+    PTFOCK_KERNEL_HSE = 1
+};
+
+enum {
+    PTFOCK_OK = 0,
+    PTFOCK_ERR_INVALID_ARG = -1,        /* null pointer, negative count, n_targets > max_targets, bad enum ... */
+    PTFOCK_ERR_UNSUPPORTED_GRID = -2,   /* a grid edge outside {16, 32, 48, 64, 128} or a slab shape with no kernel */
+    PTFOCK_ERR_UNSUPPORTED_DEVICE = -3, /* device is not compute capability 10.x */
+    PTFOCK_ERR_ALIGNMENT = -4,          /* an orbital pointer is not 16-byte aligned */
+    PTFOCK_ERR_ALLOC = -5,              /* device or host allocation failed (workspace too small included) */
+    PTFOCK_ERR_CUDA = -6,               /* a CUDA runtime call failed; see ptfock_last_cuda_error */
+    PTFOCK_ERR_ALIAS = -7               /* out overlaps phi or psi */
+};
+
+typedef struct {
+    double cell[9];           /* rows = lattice vectors a0, a1, a2 in bohr                                  */
+    int32_t n[3];             /* grid; each edge in {16, 32, 48, 64, 128}; index = (x0*n1 + x1)*n2 + x2     */
+    int32_t n_occ;            /* number of Phi orbitals (N_i of Eq. 3's sum), >= 1                         */
+    int32_t max_targets;      /* largest n_targets one apply will be given (sizes the host-path staging)   */
+    int32_t kernel;           /* PTFOCK_KERNEL_*                                                            */
+    double omega;             /* bohr^-1; HSE only                                                          */
+    double alpha;             /* mixing fraction multiplying V_X; 1.0 in all BASELINE configs */
+    int32_t device;           /* CUDA ordinal                                                               */
+    int32_t block_i;          /* pair-scheduler tile: orbitals i per wave (0 = library chooses)            */
+    int32_t block_j;          /* pair-scheduler tile: targets j per wave  (0 = library chooses)            */
+    uint64_t workspace_bytes; /* upper bound for the pair-density scratch (0 = library chooses)            */
+} ptfock_desc;
+
+/* Builds the plan: v(G) table (with -alpha/N folded in, stored in the kernels' digit-permuted
+ * frequency order), twiddle tables, scratch for one wave of pair densities.  *out is written only
+ * on success.  Synchronous. */
+int ptfock_create(const ptfock_desc *desc, ptfock_plan **out);
+
+/* out[j] = V_X[Phi] psi_j for j = 0 .. n_targets-1 (overwritten; Alg. 2 line 1 zero-initialises).
+ *   phi : n_occ grids.
+ *   psi : n_targets grids, or NULL meaning Psi = Phi[self_offset : self_offset + n_targets]
+ *         (when that range is all of Phi the scheduler uses the rho_ji = conj(rho_ij) pair symmetry).
+ *   out : n_targets grids; must not overlap phi or psi.
+ * The caller owns all three and keeps them alive until `stream` has passed the call.
+ * Asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream). */
+int ptfock_apply(ptfock_plan *plan, const void *phi, const void *psi, int32_t self_offset,
+                 int32_t n_targets, void *out, void *stream);
+
+/* E_x = 1/2 * (Omega/N) * Re sum_j sum_r conj(psi_j(r)) (V_X[Phi] psi_j)(r)   ("total energy
+ * evaluation"; reading Q11).  vx_psi: a previous ptfock_apply result for the same arguments, or
+ * NULL (the library applies into its own buffer first).  Writes one double to HOST memory *e_host and
+ * synchronises `stream`. */
+int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const void *psi, int32_t self_offset,
+                           int32_t n_targets, const void *vx_psi, double *e_host, void *stream);
+
+/* Same as ptfock_apply but phi, psi, out are HOST pointers (pinned memory gives full PCIe speed;
+ * pageable works).  The library copies Phi (and Psi) to device buffers it owns, applies, copies the
+ * result back, and synchronises `stream`.  n_targets <= max_targets. */
+int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const void *psi_host, int32_t self_offset,
+                      int32_t n_targets, void *out_host, void *stream);
+
+/* Frees everything the plan owns.  NULL is allowed. */
+int ptfock_destroy(ptfock_plan *plan);
+
+/* Static string for an error code. */
+const char *ptfock_strerror(int code);
+
+/* The cudaError_t of the most recent PTFOCK_ERR_CUDA on this thread (0 if none). */
+int ptfock_last_cuda_error(void);
+
+/* Introspection for the harness (host memory, no device work):
+ *   info[0] = block_i, info[1] = block_j in use, info[2] = scratch bytes, info[3] = kernel launches
+ *   issued by the most recent apply, info[4] = pair-solves executed by the most recent apply,
+ *   info[5] = 1 if the most recent apply used the symmetric schedule, info[6] = total launches since create,
+ *   info[7] = reserved. */
+int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]);
+
+/* Test hook: W = IFFT[v' * FFT(conj(phi_i) psi_j)] for ONE pair through the same three kernels,
+ * v' = -alpha/N * v (so V_X psi_j = sum_i phi_i W_ij).  w_out: one grid, device.  Asynchronous. */
+int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const void *psi_j, void *w_out, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PTFOCK_H */

@@ -1,0 +1,225 @@
+"""Thin Python face of the C ABI in ``include/ptfock.h`` (argument marshalling only).
+
+Every step of the path runs in the hand-written kernels of ``libptfock.so``; torch is used for device
+memory and the stream handle.  There is no CPU fallback: if the library is missing or the device is
+not a B200-class GPU the calls raise.  Operation: PAPER.md:57-61 (Eq. 3), PAPER.md:116-144 (Alg. 2).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_ROOT = os.path.dirname(_HERE)
+LIB_PATH = os.path.join(_HERE, "libptfock.so")
+SRC_DIR = os.path.join(_HERE, "csrc")
+
+KERNEL_COULOMB = 0
+KERNEL_HSE = 1
+
+EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
+           "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair"]
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+
+class PtfockError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {code}")
+        self.code = code
+
+
+class Desc(ctypes.Structure):
+    _fields_ = [("cell", ctypes.c_double * 9), ("n", ctypes.c_int32 * 3), ("n_occ", ctypes.c_int32),
+                ("max_targets", ctypes.c_int32), ("kernel", ctypes.c_int32), ("omega", ctypes.c_double),
+                ("alpha", ctypes.c_double), ("device", ctypes.c_int32), ("block_i", ctypes.c_int32),
+                ("block_j", ctypes.c_int32), ("workspace_bytes", ctypes.c_uint64)]
+
+
+def build_library(force: bool = False, verbose: bool = False) -> str:
+    """nvcc -> paper_1905_01348_b200/libptfock.so (sm_100a only, built in-tree)."""
+    srcs = [os.path.join(SRC_DIR, f) for f in sorted(os.listdir(SRC_DIR))]
+    hdr = os.path.join(_ROOT, "include", "ptfock.h")
+    newest = max(os.path.getmtime(f) for f in srcs + [hdr])
+    if not force and os.path.exists(LIB_PATH) and os.path.getmtime(LIB_PATH) >= newest:
+        return LIB_PATH
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB_PATH, os.path.join(SRC_DIR, "ptfock.cu")]
+    subprocess.run(cmd, check=True)
+    return LIB_PATH
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libptfock.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} is missing: run __graft_entry__.build() (nvcc, sm_100a); "
+                                    "there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32 = ctypes.c_void_p, ctypes.c_int32
+        L.ptfock_create.argtypes = [ctypes.POINTER(Desc), ctypes.POINTER(vp)]
+        L.ptfock_apply.argtypes = [vp, vp, vp, i32, i32, vp, vp]
+        L.ptfock_exchange_energy.argtypes = [vp, vp, vp, i32, i32, vp, ctypes.POINTER(ctypes.c_double), vp]
+        L.ptfock_apply_host.argtypes = [vp, vp, vp, i32, i32, vp, vp]
+        L.ptfock_destroy.argtypes = [vp]
+        L.ptfock_strerror.argtypes = [ctypes.c_int]
+        L.ptfock_strerror.restype = ctypes.c_char_p
+        L.ptfock_last_cuda_error.argtypes = []
+        L.ptfock_plan_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
+        L.ptfock_debug_pair.argtypes = [vp, vp, vp, vp, vp]
+        for name in EXPORTS:
+            if name != "ptfock_strerror":
+                getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        L = lib()
+        msg = L.ptfock_strerror(rc).decode()
+        if rc == -6:
+            msg += f" [cudaError {L.ptfock_last_cuda_error()}]"
+        raise PtfockError(rc, f"{what}: {msg}")
+
+
+def _dev_ptr(t, what: str, device_index: int):
+    import torch
+    if t is None:
+        return ctypes.c_void_p(0)
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()):
+        raise TypeError(f"{what} must be a contiguous complex128 CUDA tensor")
+    if t.device.index != device_index:
+        raise ValueError(f"{what} is on {t.device}, the plan is on cuda:{device_index}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host_ptr(t, what: str):
+    import torch
+    if t is None:
+        return ctypes.c_void_p(0)
+    if not (isinstance(t, torch.Tensor) and (not t.is_cuda) and t.dtype == torch.complex128 and t.is_contiguous()):
+        raise TypeError(f"{what} must be a contiguous complex128 CPU tensor")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(device_index: int):
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream(device_index).cuda_stream)
+
+
+class Plan:
+    """ptfock_create / ptfock_destroy.  ``cell``: 9 doubles (rows = lattice vectors, bohr)."""
+
+    def __init__(self, cell, n, n_occ: int, max_targets: int | None = None, kernel: int = KERNEL_HSE,
+                 omega: float = 0.106, alpha: float = 1.0, device: int = 0, block_i: int = 0, block_j: int = 0,
+                 workspace_bytes: int = 0):
+        d = Desc()
+        cell = [float(x) for x in cell]
+        if len(cell) != 9 or len(n) != 3:
+            raise ValueError("cell needs 9 numbers and n needs 3")
+        d.cell = (ctypes.c_double * 9)(*cell)
+        d.n = (ctypes.c_int32 * 3)(*[int(x) for x in n])
+        d.n_occ = int(n_occ)
+        d.max_targets = int(n_occ if max_targets is None else max_targets)
+        d.kernel, d.omega, d.alpha, d.device = int(kernel), float(omega), float(alpha), int(device)
+        d.block_i, d.block_j, d.workspace_bytes = int(block_i), int(block_j), int(workspace_bytes)
+        self._h = ctypes.c_void_p(0)
+        self.n = tuple(int(x) for x in n)
+        self.N = self.n[0] * self.n[1] * self.n[2]
+        self.n_occ = d.n_occ
+        self.device = d.device
+        _check(lib().ptfock_create(ctypes.byref(d), ctypes.byref(self._h)), "ptfock_create")
+
+    def _grids(self, t, what):
+        if t.numel() % self.N:
+            raise ValueError(f"{what} does not hold whole grids")
+        return t.numel() // self.N
+
+    def apply(self, phi, psi=None, out=None, self_offset: int = 0, n_targets: int | None = None):
+        """out[j] = V_X[phi] psi_j.  psi None: targets are phi[self_offset : self_offset + n_targets]."""
+        import torch
+        if self._grids(phi, "phi") != self.n_occ:
+            raise ValueError("phi must hold n_occ grids")
+        if psi is not None:
+            nt = self._grids(psi, "psi")
+            if n_targets is not None and n_targets != nt:
+                raise ValueError("n_targets disagrees with psi")
+        else:
+            nt = self.n_occ - self_offset if n_targets is None else n_targets
+        if out is None:
+            out = torch.empty((nt,) + self.n, dtype=torch.complex128, device=phi.device)
+        elif self._grids(out, "out") < nt:
+            raise ValueError("out is too small")
+        _check(lib().ptfock_apply(self._h, _dev_ptr(phi, "phi", self.device), _dev_ptr(psi, "psi", self.device),
+                                  int(self_offset), int(nt), _dev_ptr(out, "out", self.device), _stream(self.device)),
+               "ptfock_apply")
+        return out
+
+    def exchange_energy(self, phi, psi=None, vx_psi=None, self_offset: int = 0, n_targets: int | None = None) -> float:
+        if psi is not None:
+            nt = self._grids(psi, "psi")
+        else:
+            nt = self.n_occ - self_offset if n_targets is None else n_targets
+        e = ctypes.c_double(0.0)
+        _check(lib().ptfock_exchange_energy(self._h, _dev_ptr(phi, "phi", self.device),
+                                            _dev_ptr(psi, "psi", self.device), int(self_offset), int(nt),
+                                            _dev_ptr(vx_psi, "vx_psi", self.device), ctypes.byref(e),
+                                            _stream(self.device)), "ptfock_exchange_energy")
+        return e.value
+
+    def apply_host(self, phi, psi=None, out=None, self_offset: int = 0, n_targets: int | None = None):
+        """Host-buffer variant (ptfock_apply_host): CPU tensors in, CPU tensor out, copies inside the call."""
+        import torch
+        if psi is not None:
+            nt = self._grids(psi, "psi")
+        else:
+            nt = self.n_occ - self_offset if n_targets is None else n_targets
+        if out is None:
+            out = torch.empty((nt,) + self.n, dtype=torch.complex128)
+        _check(lib().ptfock_apply_host(self._h, _host_ptr(phi, "phi"), _host_ptr(psi, "psi"), int(self_offset),
+                                       int(nt), _host_ptr(out, "out"), _stream(self.device)), "ptfock_apply_host")
+        return out
+
+    def debug_pair(self, phi_i, psi_j):
+        import torch
+        w = torch.empty(self.n, dtype=torch.complex128, device=phi_i.device)
+        _check(lib().ptfock_debug_pair(self._h, _dev_ptr(phi_i, "phi_i", self.device),
+                                       _dev_ptr(psi_j, "psi_j", self.device), _dev_ptr(w, "w", self.device),
+                                       _stream(self.device)), "ptfock_debug_pair")
+        return w
+
+    def info(self) -> dict:
+        a = (ctypes.c_int64 * 8)()
+        _check(lib().ptfock_plan_info(self._h, a), "ptfock_plan_info")
+        return {"block_i": a[0], "block_j": a[1], "scratch_bytes": a[2], "last_launches": a[3], "last_pairs": a[4],
+                "last_symmetric": a[5], "total_launches": a[6]}
+
+    def destroy(self):
+        if self._h:
+            lib().ptfock_destroy(self._h)
+            self._h = ctypes.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.destroy()
+
+
+def plan_for(cfg, device: int = 0, max_targets: int | None = None, **kw) -> Plan:
+    """Plan for a ``synth.Config``."""
+    mt = max_targets if max_targets is not None else (cfg.j_block if cfg.j_block else cfg.n_occ)
+    return Plan(cfg.cell, cfg.n, cfg.n_occ, mt, cfg.kernel, cfg.omega, cfg.alpha, device, **kw)

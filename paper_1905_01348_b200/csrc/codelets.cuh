@@ -1,0 +1,128 @@
+// codelets.cuh -- register-resident radix-R complex fp64 DFT butterflies (R = 2, 3, 4, 8, 16).
+//
+// Building blocks of the hand-written FFT passes (BASELINE.json north_star (1): "radix-2/3/4/8/16
+// stages").  Each codelet transforms R values held in registers IN PLACE and leaves them in NATURAL
+// order:  v[k] <- sum_a v[a] exp(-/+ 2 pi i a k / R)   (INV = false: minus sign, forward DFT;
+// INV = true: plus sign, unnormalised inverse).  Register indices are compile-time after unrolling, so
+// "natural order" costs no data movement.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace ptfock {
+
+typedef double2 cd;
+
+#define PTF_DEV __device__ __forceinline__
+
+PTF_DEV cd cadd(cd a, cd b) { return make_double2(a.x + b.x, a.y + b.y); }
+PTF_DEV cd csub(cd a, cd b) { return make_double2(a.x - b.x, a.y - b.y); }
+PTF_DEV cd cmul(cd a, cd b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// a * conj(b)
+PTF_DEV cd cmulc(cd a, cd b) { return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
+PTF_DEV cd cconj(cd a) { return make_double2(a.x, -a.y); }
+PTF_DEV cd cscale(cd a, double s) { return make_double2(a.x * s, a.y * s); }
+
+// multiply by exp(-/+ i pi/2) = -/+ i
+template <bool INV> PTF_DEV cd mul_mi(cd a) { return INV ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x); }
+// multiply by a forward-sign twiddle w (INV: by conj(w))
+template <bool INV> PTF_DEV cd twmul(cd a, cd w) { return INV ? cmulc(a, w) : cmul(a, w); }
+
+constexpr double kSqrtHalf = 0.70710678118654752440084436210485;
+constexpr double kCosPi8 = 0.92387953251128675612818318939679;
+constexpr double kSinPi8 = 0.38268343236508977172845998403040;
+constexpr double kSin2Pi3 = 0.86602540378443864676372317075294;
+
+template <int R, bool INV> struct DFT;
+
+template <bool INV> struct DFT<1, INV> {
+    static PTF_DEV void run(cd (&)[1]) {}
+};
+
+template <bool INV> struct DFT<2, INV> {
+    static PTF_DEV void run(cd (&v)[2]) {
+        cd a = v[0], b = v[1];
+        v[0] = cadd(a, b);
+        v[1] = csub(a, b);
+    }
+};
+
+template <bool INV> struct DFT<3, INV> {
+    static PTF_DEV void run(cd (&v)[3]) {
+        cd t = cadd(v[1], v[2]);
+        cd d = csub(v[1], v[2]);
+        cd m = make_double2(v[0].x - 0.5 * t.x, v[0].y - 0.5 * t.y);
+        // u = (-/+ i) sin(2pi/3) d
+        cd u = mul_mi<INV>(cscale(d, kSin2Pi3));
+        v[0] = cadd(v[0], t);
+        v[1] = cadd(m, u);
+        v[2] = csub(m, u);
+    }
+};
+
+template <bool INV> struct DFT<4, INV> {
+    static PTF_DEV void run(cd &a0, cd &a1, cd &a2, cd &a3) {
+        cd t0 = cadd(a0, a2), t1 = csub(a0, a2);
+        cd t2 = cadd(a1, a3), t3 = mul_mi<INV>(csub(a1, a3));
+        a0 = cadd(t0, t2);
+        a2 = csub(t0, t2);
+        a1 = cadd(t1, t3);
+        a3 = csub(t1, t3);
+    }
+    static PTF_DEV void run(cd (&v)[4]) { run(v[0], v[1], v[2], v[3]); }
+};
+
+template <bool INV> struct DFT<8, INV> {
+    static PTF_DEV void run(cd (&v)[8]) {
+        // decimation in time: even / odd halves, then the w8^k combine
+        DFT<4, INV>::run(v[0], v[2], v[4], v[6]);   // E[0..3] in v[0], v[2], v[4], v[6]
+        DFT<4, INV>::run(v[1], v[3], v[5], v[7]);   // O[0..3] in v[1], v[3], v[5], v[7]
+        cd o0 = v[1];
+        // w8^1 = (1 -/+ i)/sqrt2 ; w8^2 = -/+ i ; w8^3 = (-1 -/+ i)/sqrt2
+        cd o1 = INV ? make_double2((v[3].x - v[3].y) * kSqrtHalf, (v[3].x + v[3].y) * kSqrtHalf)
+                    : make_double2((v[3].x + v[3].y) * kSqrtHalf, (v[3].y - v[3].x) * kSqrtHalf);
+        cd o2 = mul_mi<INV>(v[5]);
+        cd o3 = INV ? make_double2(-(v[7].x + v[7].y) * kSqrtHalf, (v[7].x - v[7].y) * kSqrtHalf)
+                    : make_double2((v[7].y - v[7].x) * kSqrtHalf, -(v[7].x + v[7].y) * kSqrtHalf);
+        cd e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+        v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+        v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
+        v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
+        v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
+    }
+};
+
+template <bool INV> struct DFT<16, INV> {
+    static PTF_DEV void run(cd (&v)[16]) {
+        // 16 = 4 x 4: x = 4a + b.  DFT over a for each b, twiddle w16^(b k1), DFT over b for each k1,
+        // result index k1 + 4 k2.
+#pragma unroll
+        for (int b = 0; b < 4; ++b) DFT<4, INV>::run(v[b], v[4 + b], v[8 + b], v[12 + b]);   // -> y[k1][b] at v[4 k1 + b]
+        const cd w1 = make_double2(kCosPi8, -kSinPi8);        // w16^1 (forward sign)
+        const cd w2 = make_double2(kSqrtHalf, -kSqrtHalf);    // w16^2
+        const cd w3 = make_double2(kSinPi8, -kCosPi8);        // w16^3
+        const cd w6 = make_double2(-kSqrtHalf, -kSqrtHalf);   // w16^6
+        const cd w9 = make_double2(-kCosPi8, kSinPi8);        // w16^9
+        v[4 + 1] = twmul<INV>(v[4 + 1], w1);
+        v[4 + 2] = twmul<INV>(v[4 + 2], w2);
+        v[4 + 3] = twmul<INV>(v[4 + 3], w3);
+        v[8 + 1] = twmul<INV>(v[8 + 1], w2);
+        v[8 + 2] = mul_mi<INV>(v[8 + 2]);                      // w16^4 = -/+ i
+        v[8 + 3] = twmul<INV>(v[8 + 3], w6);
+        v[12 + 1] = twmul<INV>(v[12 + 1], w3);
+        v[12 + 2] = twmul<INV>(v[12 + 2], w6);
+        v[12 + 3] = twmul<INV>(v[12 + 3], w9);
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1) DFT<4, INV>::run(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);
+        // v[4 k1 + k2] holds X[k1 + 4 k2]: transpose the 4x4 register tile (free: renaming)
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1)
+#pragma unroll
+            for (int k2 = k1 + 1; k2 < 4; ++k2) {
+                cd t = v[4 * k1 + k2];
+                v[4 * k1 + k2] = v[4 * k2 + k1];
+                v[4 * k2 + k1] = t;
+            }
+    }
+};
+
+}  // namespace ptfock

@@ -1,0 +1,525 @@
+// ptfock.cu -- host side of libptfock.so: the C ABI of include/ptfock.h, plan construction
+// (v' table, twiddles, scratch) and the pair scheduler (Alg. 2 loops i x j, batched as in
+// PAPER.md:149 "Batched implementation"; i <= j pair symmetry when Psi = Phi).
+#include "../../include/ptfock.h"
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace ptfock;
+
+namespace {
+
+thread_local int g_last_cuda = 0;
+
+#define CU(call)                                              \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) {                             \
+            g_last_cuda = (int)e__;                           \
+            return PTFOCK_ERR_CUDA;                           \
+        }                                                     \
+    } while (0)
+
+typedef void (*slab_launch_fn)(const SlabArgs &, dim3, cudaStream_t);
+typedef void (*pencil_launch_fn)(const PencilArgs &, int pairs, cudaStream_t);
+
+template <int N1, int N2> void launch_slab_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
+    slab_fwd<N1, N2><<<grid, kSlabThreads, SlabShape<N1, N2>::SMEM_BYTES, st>>>(a);
+}
+template <int N1, int N2> void launch_slab_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) {
+    slab_inv_acc<N1, N2><<<grid, kSlabThreads, SlabShape<N1, N2>::SMEM_BYTES, st>>>(a);
+}
+template <int N0> void launch_pencil(const PencilArgs &a, int pairs, cudaStream_t st) {
+    using S = PencilShape<N0>;
+    const int gx = (S::R2 == 1) ? (a.slab_pts + S::NT - 1) / S::NT : a.slab_pts / S::CW;
+    pencil_mid<N0><<<dim3(gx, pairs), S::NT, S::SMEM_BYTES, st>>>(a);
+}
+
+struct SlabEntry {
+    int n1, n2;
+    slab_launch_fn fwd, inv;
+    cudaError_t (*prepare)();
+};
+
+template <int N1, int N2> cudaError_t prepare_slab() {
+    cudaError_t e = cudaFuncSetAttribute(slab_fwd<N1, N2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         SlabShape<N1, N2>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(slab_inv_acc<N1, N2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                SlabShape<N1, N2>::SMEM_BYTES);
+}
+
+#define SLAB(N1, N2) { N1, N2, launch_slab_fwd<N1, N2>, launch_slab_inv<N1, N2>, prepare_slab<N1, N2> }
+const SlabEntry kSlabs[] = {
+    SLAB(16, 16), SLAB(32, 32), SLAB(48, 48), SLAB(64, 64), SLAB(128, 48),          // the five BASELINE configs
+    SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),           // non-square test shapes
+};
+#undef SLAB
+
+struct PencilEntry {
+    int n0;
+    pencil_launch_fn run;
+    cudaError_t (*prepare)();
+};
+template <int N0> cudaError_t prepare_pencil() {
+    if (PencilShape<N0>::SMEM_BYTES <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(pencil_mid<N0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                PencilShape<N0>::SMEM_BYTES);
+}
+#define PENCIL(N0) { N0, launch_pencil<N0>, prepare_pencil<N0> }
+const PencilEntry kPencils[] = { PENCIL(16), PENCIL(32), PENCIL(48), PENCIL(64), PENCIL(128) };
+#undef PENCIL
+
+// position -> frequency index of the digit-permuted order the forward passes leave an axis in
+int freq_of_pos(int n, int pos) {
+    int r1, r2;
+    switch (n) {
+        case 16: r1 = 16; r2 = 1; break;
+        case 32: r1 = 8; r2 = 4; break;
+        case 48: r1 = 16; r2 = 3; break;
+        case 64: r1 = 8; r2 = 8; break;
+        case 128: r1 = 16; r2 = 8; break;
+        default: return -1;
+    }
+    const int k1 = pos / r2, k2 = pos % r2;
+    return k1 + r1 * k2;
+}
+
+double det3(const double *a) {
+    return a[0] * (a[4] * a[8] - a[5] * a[7]) - a[1] * (a[3] * a[8] - a[5] * a[6]) + a[2] * (a[3] * a[7] - a[4] * a[6]);
+}
+
+__global__ void fill_ones(cd *p, long long n) {
+    long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) p[k] = make_double2(1.0, 0.0);
+}
+
+}  // namespace
+
+struct ptfock_plan {
+    ptfock_desc d;
+    long long N;
+    int slab_pts;
+    double volume;
+    double *v_dev;
+    cd *tw_dev[3];
+    cd *scratch;
+    size_t scratch_bytes;
+    int Ib, Jb;
+    bool v_even;
+    const SlabEntry *slab;
+    const PencilEntry *pencil;
+    // exchange energy
+    double2 *partials, *result_dev, *result_host;
+    cd *energy_buf;
+    // host path staging
+    cd *st_phi, *st_psi, *st_out;
+    // statistics
+    long long last_launches, last_pairs, total_launches;
+    int last_symmetric;
+};
+
+// ================================================================================================
+// plan
+// ================================================================================================
+namespace {
+
+const int kEdges[] = { 16, 32, 48, 64, 128 };
+bool edge_ok(int n) {
+    for (int e : kEdges) if (e == n) return true;
+    return false;
+}
+
+void free_plan(ptfock_plan *p) {
+    if (!p) return;
+    cudaFree(p->v_dev);
+    for (int d = 0; d < 3; ++d) cudaFree(p->tw_dev[d]);
+    cudaFree(p->scratch);
+    cudaFree(p->partials);
+    cudaFree(p->result_dev);
+    if (p->result_host) cudaFreeHost(p->result_host);
+    cudaFree(p->energy_buf);
+    cudaFree(p->st_phi);
+    cudaFree(p->st_psi);
+    cudaFree(p->st_out);
+    delete p;
+}
+
+// v'(pos0, pos1, pos2) = -alpha/N * v(|G|^2) in the permuted order; also reports whether v(-G) = v(G)
+// holds on the grid (needed by the pair-symmetric schedule; fails for skew cells at Nyquist planes).
+int build_vtable(const ptfock_desc &d, std::vector<double> &vperm, bool &even) {
+    const int n0 = d.n[0], n1 = d.n[1], n2 = d.n[2];
+    const long long N = (long long)n0 * n1 * n2;
+    const double *a = d.cell;
+    const double vol = det3(a);
+    if (vol == 0.0 || !std::isfinite(vol)) return PTFOCK_ERR_INVALID_ARG;
+    const double two_pi = 6.283185307179586476925286766559;
+    const double f = two_pi / vol;
+    // reciprocal rows b_d = 2 pi (a_e x a_f) / vol
+    double b[9];
+    b[0] = f * (a[4] * a[8] - a[5] * a[7]); b[1] = f * (a[5] * a[6] - a[3] * a[8]); b[2] = f * (a[3] * a[7] - a[4] * a[6]);
+    b[3] = f * (a[7] * a[2] - a[8] * a[1]); b[4] = f * (a[8] * a[0] - a[6] * a[2]); b[5] = f * (a[6] * a[1] - a[7] * a[0]);
+    b[6] = f * (a[1] * a[5] - a[2] * a[4]); b[7] = f * (a[2] * a[3] - a[0] * a[5]); b[8] = f * (a[0] * a[4] - a[1] * a[3]);
+    std::vector<double> vnat((size_t)N);
+    const double four_pi = 2.0 * two_pi;
+    const double inv4w2 = (d.kernel == PTFOCK_KERNEL_HSE) ? 1.0 / (4.0 * d.omega * d.omega) : 0.0;
+    for (int k0 = 0; k0 < n0; ++k0) {
+        const int m0 = (k0 < n0 / 2) ? k0 : k0 - n0;
+        for (int k1 = 0; k1 < n1; ++k1) {
+            const int m1 = (k1 < n1 / 2) ? k1 : k1 - n1;
+            for (int k2 = 0; k2 < n2; ++k2) {
+                const int m2 = (k2 < n2 / 2) ? k2 : k2 - n2;
+                const double gx = m0 * b[0] + m1 * b[3] + m2 * b[6];
+                const double gy = m0 * b[1] + m1 * b[4] + m2 * b[7];
+                const double gz = m0 * b[2] + m1 * b[5] + m2 * b[8];
+                const double g2 = gx * gx + gy * gy + gz * gz;
+                double val;
+                if ((m0 | m1 | m2) == 0)
+                    val = (d.kernel == PTFOCK_KERNEL_HSE) ? 0.5 * two_pi / (d.omega * d.omega) : 0.0;
+                else if (d.kernel == PTFOCK_KERNEL_HSE)
+                    val = four_pi / g2 * (-std::expm1(-g2 * inv4w2));
+                else
+                    val = four_pi / g2;
+                vnat[((size_t)k0 * n1 + k1) * n2 + k2] = val;
+            }
+        }
+    }
+    even = true;
+    for (int k0 = 0; k0 < n0 && even; ++k0)
+        for (int k1 = 0; k1 < n1 && even; ++k1)
+            for (int k2 = 0; k2 < n2; ++k2) {
+                const double x = vnat[((size_t)k0 * n1 + k1) * n2 + k2];
+                const double y = vnat[((size_t)((n0 - k0) % n0) * n1 + (n1 - k1) % n1) * n2 + (n2 - k2) % n2];
+                if (std::fabs(x - y) > 1e-14 * (std::fabs(x) + std::fabs(y))) { even = false; break; }
+            }
+    const double scale = -d.alpha / (double)N;
+    vperm.resize((size_t)N);
+    for (int p0 = 0; p0 < n0; ++p0) {
+        const int k0 = freq_of_pos(n0, p0);
+        for (int p1 = 0; p1 < n1; ++p1) {
+            const int k1 = freq_of_pos(n1, p1);
+            for (int p2 = 0; p2 < n2; ++p2) {
+                const int k2 = freq_of_pos(n2, p2);
+                vperm[((size_t)p0 * n1 + p1) * n2 + p2] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
+            }
+        }
+    }
+    return PTFOCK_OK;
+}
+
+}  // namespace
+
+extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
+    if (!desc || !out) return PTFOCK_ERR_INVALID_ARG;
+    const ptfock_desc &d = *desc;
+    if (d.n_occ < 1 || d.max_targets < 1 || d.block_i < 0 || d.block_j < 0) return PTFOCK_ERR_INVALID_ARG;
+    if (d.kernel != PTFOCK_KERNEL_COULOMB && d.kernel != PTFOCK_KERNEL_HSE) return PTFOCK_ERR_INVALID_ARG;
+    if (d.kernel == PTFOCK_KERNEL_HSE && !(d.omega > 0.0)) return PTFOCK_ERR_INVALID_ARG;
+    if (!std::isfinite(d.alpha)) return PTFOCK_ERR_INVALID_ARG;
+    for (int k = 0; k < 3; ++k) if (!edge_ok(d.n[k])) return PTFOCK_ERR_UNSUPPORTED_GRID;
+    const SlabEntry *slab = nullptr;
+    for (const SlabEntry &e : kSlabs) if (e.n1 == d.n[1] && e.n2 == d.n[2]) slab = &e;
+    const PencilEntry *pencil = nullptr;
+    for (const PencilEntry &e : kPencils) if (e.n0 == d.n[0]) pencil = &e;
+    if (!slab || !pencil) return PTFOCK_ERR_UNSUPPORTED_GRID;
+    if (det3(d.cell) == 0.0) return PTFOCK_ERR_INVALID_ARG;
+
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    if (d.device < 0 || d.device >= ndev) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, d.device));
+    if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;     // sm_100a code only, no fallback
+    CU(cudaSetDevice(d.device));
+
+    ptfock_plan *p = new (std::nothrow) ptfock_plan();
+    if (!p) return PTFOCK_ERR_ALLOC;
+    std::memset(p, 0, sizeof(*p));
+    p->d = d;
+    p->N = (long long)d.n[0] * d.n[1] * d.n[2];
+    p->slab_pts = d.n[1] * d.n[2];
+    p->volume = std::fabs(det3(d.cell));
+    p->slab = slab;
+    p->pencil = pencil;
+
+    std::vector<double> vperm;
+    bool even = false;
+    int rc = build_vtable(d, vperm, even);
+    if (rc != PTFOCK_OK) { free_plan(p); return rc; }
+    p->v_even = even;
+
+#define CUP(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_cuda = (int)e__; free_plan(p); \
+        return (e__ == cudaErrorMemoryAllocation) ? PTFOCK_ERR_ALLOC : PTFOCK_ERR_CUDA; } } while (0)
+
+    CUP(slab->prepare());
+    CUP(pencil->prepare());
+    CUP(cudaMalloc(&p->v_dev, sizeof(double) * p->N));
+    CUP(cudaMemcpy(p->v_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
+    for (int k = 0; k < 3; ++k) {
+        const int n = d.n[k];
+        std::vector<cd> tw((size_t)n);
+        for (int t = 0; t < n; ++t) {
+            const long double ang = 2.0L * 3.14159265358979323846264338327950288L * (long double)t / (long double)n;
+            tw[t] = make_double2((double)cosl(ang), (double)(-sinl(ang)));     // exp(-2 pi i t / n)
+        }
+        CUP(cudaMalloc(&p->tw_dev[k], sizeof(cd) * n));
+        CUP(cudaMemcpy(p->tw_dev[k], tw.data(), sizeof(cd) * n, cudaMemcpyHostToDevice));
+    }
+    // pair-scheduler tile
+    int Ib = d.block_i > 0 ? d.block_i : 16;
+    int Jb = d.block_j > 0 ? d.block_j : 8;
+    if (Ib > d.n_occ) Ib = d.n_occ;
+    if (Jb > d.max_targets) Jb = d.max_targets;
+    const size_t pair_bytes = sizeof(cd) * (size_t)p->N;
+    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)2 << 30);
+    while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
+    while ((size_t)Ib * Jb * pair_bytes > limit && Jb > 1) Jb = (Jb + 1) / 2;
+    if ((size_t)Ib * Jb * pair_bytes > limit) { free_plan(p); return PTFOCK_ERR_ALLOC; }
+    p->Ib = Ib;
+    p->Jb = Jb;
+    p->scratch_bytes = (size_t)Ib * Jb * pair_bytes;
+    CUP(cudaMalloc(&p->scratch, p->scratch_bytes));
+    CUP(cudaMalloc(&p->partials, sizeof(double2) * 1024));
+    CUP(cudaMalloc(&p->result_dev, sizeof(double2)));
+    CUP(cudaMallocHost(&p->result_host, sizeof(double2)));
+#undef CUP
+    *out = p;
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_destroy(ptfock_plan *plan) {
+    if (!plan) return PTFOCK_OK;
+    cudaSetDevice(plan->d.device);
+    cudaDeviceSynchronize();
+    free_plan(plan);
+    return PTFOCK_OK;
+}
+
+extern "C" const char *ptfock_strerror(int code) {
+    switch (code) {
+        case PTFOCK_OK: return "ok";
+        case PTFOCK_ERR_INVALID_ARG: return "invalid argument";
+        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (edges must be in {16,32,48,64,128} with a built slab shape)";
+        case PTFOCK_ERR_UNSUPPORTED_DEVICE: return "unsupported device (needs compute capability 10.x; there is no CPU fallback)";
+        case PTFOCK_ERR_ALIGNMENT: return "pointer not 16-byte aligned";
+        case PTFOCK_ERR_ALLOC: return "allocation failed or workspace too small";
+        case PTFOCK_ERR_CUDA: return "CUDA runtime error (see ptfock_last_cuda_error)";
+        case PTFOCK_ERR_ALIAS: return "out overlaps an input";
+        default: return "unknown error";
+    }
+}
+
+extern "C" int ptfock_last_cuda_error(void) { return g_last_cuda; }
+
+extern "C" int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]) {
+    if (!plan || !info) return PTFOCK_ERR_INVALID_ARG;
+    info[0] = plan->Ib;
+    info[1] = plan->Jb;
+    info[2] = (int64_t)plan->scratch_bytes;
+    info[3] = plan->last_launches;
+    info[4] = plan->last_pairs;
+    info[5] = plan->last_symmetric;
+    info[6] = plan->total_launches;
+    info[7] = 0;
+    return PTFOCK_OK;
+}
+
+// ================================================================================================
+// pair scheduler
+// ================================================================================================
+namespace {
+
+struct Wave {
+    ptfock_plan *p;
+    cudaStream_t st;
+    long long launches, pairs;
+};
+
+// A + B for the block of pairs (i in [i0, i0+ni)) x (j in [j0, j0+nj)); pair index = ii * nj + jj.
+void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int j0, int nj) {
+    ptfock_plan *p = w.p;
+    SlabArgs a;
+    a.a = phi; a.b = psi; a.scratch = p->scratch; a.out = nullptr;
+    a.tw1 = p->tw_dev[1]; a.tw2 = p->tw_dev[2];
+    a.grid_pts = p->N; a.n0 = p->d.n[0];
+    a.a0 = i0; a.na = ni; a.b0 = j0;
+    a.stride_loop = nj; a.stride_cta = 1; a.conj_w = 0;
+    // split the i loop over blockIdx.z until the grid has a few CTAs per SM
+    int z = 1;
+    const long long base = (long long)p->d.n[0] * nj;
+    while (z < ni && base * z < 148LL * 6) z *= 2;
+    if (z > ni) z = ni;
+    p->slab->fwd(a, dim3(p->d.n[0], nj, z), w.st);
+    PencilArgs b;
+    b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
+    p->pencil->run(b, ni * nj, w.st);
+    w.launches += 2;
+    w.pairs += (long long)ni * nj;
+}
+
+// C: out[t0 + tt] += sum_ss orb[s0 + ss] * W(ss, tt)
+void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, int nt, int stride_loop, int stride_cta,
+                     int conj_w) {
+    ptfock_plan *p = w.p;
+    SlabArgs a;
+    a.a = orb; a.b = nullptr; a.scratch = p->scratch; a.out = out;
+    a.tw1 = p->tw_dev[1]; a.tw2 = p->tw_dev[2];
+    a.grid_pts = p->N; a.n0 = p->d.n[0];
+    a.a0 = s0; a.na = ns; a.b0 = t0;
+    a.stride_loop = stride_loop; a.stride_cta = stride_cta; a.conj_w = conj_w;
+    p->slab->inv(a, dim3(p->d.n[0], nt, 1), w.st);
+    w.launches += 1;
+}
+
+bool overlaps(const void *a, size_t na, const void *b, size_t nb) {
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    return x < y + nb && y < x + na;
+}
+
+int check_apply_args(const ptfock_plan *p, const void *phi, const void *psi, int self_offset, int n_targets,
+                     const void *out) {
+    if (!p || !phi || n_targets < 0) return PTFOCK_ERR_INVALID_ARG;
+    if (!out && n_targets > 0) return PTFOCK_ERR_INVALID_ARG;
+    if (!psi && (self_offset < 0 || (long long)self_offset + n_targets > p->d.n_occ)) return PTFOCK_ERR_INVALID_ARG;
+    if (((uintptr_t)phi | (uintptr_t)psi | (uintptr_t)out) & 15) return PTFOCK_ERR_ALIGNMENT;
+    return PTFOCK_OK;
+}
+
+int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, int n_targets, cd *out,
+                 cudaStream_t st) {
+    const size_t gbytes = sizeof(cd) * (size_t)p->N;
+    if (n_targets == 0) { p->last_launches = 0; p->last_pairs = 0; p->last_symmetric = 0; return PTFOCK_OK; }
+    if (overlaps(out, gbytes * n_targets, phi, gbytes * p->d.n_occ)) return PTFOCK_ERR_ALIAS;
+    if (psi && overlaps(out, gbytes * n_targets, psi, gbytes * n_targets)) return PTFOCK_ERR_ALIAS;
+    CU(cudaSetDevice(p->d.device));
+    CU(cudaMemsetAsync(out, 0, gbytes * n_targets, st));             // Alg. 2 line 1
+    Wave w{ p, st, 0, 0 };
+    const int n_occ = p->d.n_occ;
+    const bool symmetric = (!psi) && self_offset == 0 && n_targets == n_occ && p->v_even && n_occ > 1;
+    if (symmetric) {
+        // square blocks; block pair (bi <= bj): W_ij for i in bi, j in bj serves out_j (as is) and, off the
+        // diagonal, out_i through W_ji = conj(W_ij) (v real and even).
+        int bs = p->Ib < p->Jb ? p->Ib : p->Jb;
+        while ((size_t)(bs * 2) * (bs * 2) * gbytes <= p->scratch_bytes && bs * 2 <= n_occ) bs *= 2;
+        for (int j0 = 0; j0 < n_occ; j0 += bs) {
+            const int nj = (n_occ - j0 < bs) ? n_occ - j0 : bs;
+            for (int i0 = 0; i0 <= j0; i0 += bs) {
+                const int ni = (n_occ - i0 < bs) ? n_occ - i0 : bs;
+                wave_forward_mid(w, phi, phi, i0, ni, j0, nj);
+                wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
+                if (i0 != j0) wave_accumulate(w, phi, j0, nj, out, i0, ni, 1, nj, 1);
+            }
+        }
+    } else {
+        const cd *tgt = psi ? psi : phi + (size_t)self_offset * p->N;
+        for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
+            const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
+            for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
+                const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
+                wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
+                wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
+            }
+        }
+    }
+    CU(cudaGetLastError());
+    p->last_launches = w.launches;
+    p->last_pairs = w.pairs;
+    p->last_symmetric = symmetric ? 1 : 0;
+    p->total_launches += w.launches;
+    return PTFOCK_OK;
+}
+
+}  // namespace
+
+extern "C" int ptfock_apply(ptfock_plan *plan, const void *phi, const void *psi, int32_t self_offset,
+                            int32_t n_targets, void *out, void *stream) {
+    int rc = check_apply_args(plan, phi, psi, self_offset, n_targets, out);
+    if (rc != PTFOCK_OK) return rc;
+    return apply_device(plan, (const cd *)phi, (const cd *)psi, self_offset, n_targets, (cd *)out, (cudaStream_t)stream);
+}
+
+extern "C" int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const void *psi, int32_t self_offset,
+                                      int32_t n_targets, const void *vx_psi, double *e_host, void *stream) {
+    if (!plan || !phi || !e_host || n_targets < 0) return PTFOCK_ERR_INVALID_ARG;
+    if (!psi && (self_offset < 0 || (long long)self_offset + n_targets > plan->d.n_occ)) return PTFOCK_ERR_INVALID_ARG;
+    if (((uintptr_t)phi | (uintptr_t)psi | (uintptr_t)vx_psi) & 15) return PTFOCK_ERR_ALIGNMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaSetDevice(plan->d.device));
+    if (n_targets == 0) { *e_host = 0.0; return PTFOCK_OK; }
+    const cd *vx = (const cd *)vx_psi;
+    if (!vx) {
+        if (n_targets > plan->d.max_targets) return PTFOCK_ERR_INVALID_ARG;
+        if (!plan->energy_buf) {
+            cudaError_t e = cudaMalloc(&plan->energy_buf, sizeof(cd) * (size_t)plan->N * plan->d.max_targets);
+            if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
+        }
+        int rc = apply_device(plan, (const cd *)phi, (const cd *)psi, self_offset, n_targets, plan->energy_buf, st);
+        if (rc != PTFOCK_OK) return rc;
+        vx = plan->energy_buf;
+    }
+    const cd *tgt = psi ? (const cd *)psi : (const cd *)phi + (size_t)self_offset * plan->N;
+    const long long n = plan->N * (long long)n_targets;
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > 1024) blocks = 1024;
+    dot_partial<<<blocks, 256, 0, st>>>(tgt, vx, n, plan->partials);
+    dot_final<<<1, 256, 0, st>>>(plan->partials, blocks, 0.5 * plan->volume / (double)plan->N, plan->result_dev);
+    plan->total_launches += 2;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(plan->result_host, plan->result_dev, sizeof(double2), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    *e_host = plan->result_host->x;
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const void *psi_host, int32_t self_offset,
+                                 int32_t n_targets, void *out_host, void *stream) {
+    if (!plan || !phi_host || !out_host || n_targets < 0 || n_targets > plan->d.max_targets) return PTFOCK_ERR_INVALID_ARG;
+    if (!psi_host && (self_offset < 0 || (long long)self_offset + n_targets > plan->d.n_occ)) return PTFOCK_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaSetDevice(plan->d.device));
+    const size_t gbytes = sizeof(cd) * (size_t)plan->N;
+    auto ensure = [&](cd **buf, size_t bytes) -> int {
+        if (*buf) return PTFOCK_OK;
+        cudaError_t e = cudaMalloc(buf, bytes);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
+        return PTFOCK_OK;
+    };
+    int rc = ensure(&plan->st_phi, gbytes * plan->d.n_occ);
+    if (rc == PTFOCK_OK) rc = ensure(&plan->st_out, gbytes * plan->d.max_targets);
+    if (rc == PTFOCK_OK && psi_host) rc = ensure(&plan->st_psi, gbytes * plan->d.max_targets);
+    if (rc != PTFOCK_OK) return rc;
+    CU(cudaMemcpyAsync(plan->st_phi, phi_host, gbytes * plan->d.n_occ, cudaMemcpyHostToDevice, st));
+    if (psi_host) CU(cudaMemcpyAsync(plan->st_psi, psi_host, gbytes * n_targets, cudaMemcpyHostToDevice, st));
+    rc = apply_device(plan, plan->st_phi, psi_host ? plan->st_psi : nullptr, self_offset, n_targets, plan->st_out, st);
+    if (rc != PTFOCK_OK) return rc;
+    CU(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const void *psi_j, void *w_out, void *stream) {
+    if (!plan || !phi_i || !psi_j || !w_out) return PTFOCK_ERR_INVALID_ARG;
+    if (((uintptr_t)phi_i | (uintptr_t)psi_j | (uintptr_t)w_out) & 15) return PTFOCK_ERR_ALIGNMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaSetDevice(plan->d.device));
+    const size_t gbytes = sizeof(cd) * (size_t)plan->N;
+    cd *ones = nullptr;
+    cudaError_t e = cudaMalloc(&ones, gbytes);
+    if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
+    fill_ones<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(ones, plan->N);
+    cudaMemsetAsync(w_out, 0, gbytes, st);
+    Wave w{ plan, st, 0, 0 };
+    wave_forward_mid(w, (const cd *)phi_i, (const cd *)psi_j, 0, 1, 0, 1);
+    wave_accumulate(w, ones, 0, 1, (cd *)w_out, 0, 1, 1, 1, 0);
+    plan->total_launches += w.launches + 1;
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaFree(ones);
+    if (e2 != cudaSuccess) { g_last_cuda = (int)e2; return PTFOCK_ERR_CUDA; }
+    return PTFOCK_OK;
+}

@@ -1,0 +1,146 @@
+"""GPU vs oracle parity (T9 of SURVEY.md 8(c)): every call goes through the C ABI (binding -> libptfock.so).
+
+Bar (BASELINE.json north_star): max_{j,r} |gpu - ref| / max_{j,r} |ref| <= 1e-10.  The transforms are exact
+circular convolutions in fp64, so the observed error is ~1e-15..1e-13.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1905_01348_b200 import binding, synth
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def _rel(got, ref):
+    return float(np.abs(got - ref).max() / np.abs(ref).max())
+
+
+def _oracle(cfg, phi, psi=None, cols=None):
+    return oracle.apply(cfg.cell, cfg.n, cfg.kernel, cfg.omega, cfg.alpha, phi.cpu().numpy(),
+                        None if psi is None else psi.cpu().numpy(), cols)
+
+
+SMALL = [
+    # name, edges, grid, n_occ, kernel, separate psi
+    ("c16", (10.26,) * 3, (16, 16, 16), 5, synth.KERNEL_HSE, False),
+    ("c16ns", (10.26,) * 3, (16, 16, 16), 5, synth.KERNEL_COULOMB, True),
+    ("g16x32x16", (9.0, 17.0, 12.0), (16, 32, 16), 4, synth.KERNEL_HSE, True),
+    ("g32x16x32", (15.0, 9.0, 17.0), (32, 16, 32), 3, synth.KERNEL_COULOMB, False),
+    ("g48x16x48", (22.0, 9.0, 23.0), (48, 16, 48), 3, synth.KERNEL_HSE, True),
+    ("g64x48x32", (30.0, 22.0, 16.0), (64, 48, 32), 2, synth.KERNEL_HSE, True),
+    ("g128x32x64", (50.0, 16.0, 30.0), (128, 32, 64), 2, synth.KERNEL_HSE, True),
+    ("g32x128x48", (16.0, 50.0, 22.0), (32, 128, 48), 2, synth.KERNEL_COULOMB, False),
+]
+
+
+@pytest.mark.parametrize("case", SMALL, ids=[c[0] for c in SMALL])
+def test_small_grids_every_codelet(cuda_device, case):
+    """Every supported edge length on every axis role (pencil x0, slab x1, slab x2), noise inputs."""
+    name, edges, n, n_occ, kernel, sep = case
+    cfg = synth.Config(name, edges, n, n_occ, kernel, separate_psi=sep)
+    phi = synth.random_orbitals(cfg, 11, n_occ, cuda_device)
+    psi = synth.random_orbitals(cfg, 12, 3, cuda_device) if sep else None
+    with binding.plan_for(cfg, block_i=2, block_j=2) as plan:
+        out = plan.apply(phi, psi)
+        torch.cuda.synchronize()
+    assert _rel(out.cpu().numpy(), _oracle(cfg, phi, psi)) <= TOL
+
+
+def test_debug_pair_matches_oracle_W(cuda_device):
+    cfg = synth.Config("w", (9.0, 17.0, 12.0), (16, 32, 16), 2, synth.KERNEL_HSE, alpha=0.25)
+    ab = synth.random_orbitals(cfg, 5, 2, cuda_device)
+    with binding.plan_for(cfg) as plan:
+        w = plan.debug_pair(ab[0], ab[1]).cpu().numpy()
+    ref = -cfg.alpha * oracle.pair_w(cfg.cell, cfg.n, cfg.kernel, cfg.omega, ab[0].cpu().numpy(), ab[1].cpu().numpy())
+    assert _rel(w, ref) <= TOL
+
+
+def test_Si8_full(cuda_device):
+    cfg = synth.CONFIGS["Si8"]
+    phi = synth.orbitals(cfg, device=cuda_device)
+    with binding.plan_for(cfg) as plan:
+        out = plan.apply(phi)
+        e = plan.exchange_energy(phi, vx_psi=out)
+        e2 = plan.exchange_energy(phi)
+        info = plan.info()
+    assert info["last_symmetric"] == 1
+    ref = _oracle(cfg, phi)
+    assert _rel(out.cpu().numpy(), ref) <= TOL
+    e_ref = oracle.exchange_energy(cfg.cell, cfg.n, phi.cpu().numpy(), ref)
+    assert abs(e - e_ref.real) <= TOL * abs(e_ref.real) and abs(e2 - e_ref.real) <= TOL * abs(e_ref.real)
+    assert e < 0.0
+
+
+def test_Si64_full(cuda_device):
+    cfg = synth.CONFIGS["Si64"]
+    phi = synth.orbitals(cfg, device=cuda_device)
+    with binding.plan_for(cfg) as plan:
+        out = plan.apply(phi)
+        torch.cuda.synchronize()
+        assert plan.info()["last_symmetric"] == 1
+    assert _rel(out.cpu().numpy(), _oracle(cfg, phi)) <= TOL
+
+
+def test_schedules_agree(cuda_device):
+    """Symmetric schedule == general schedule on a copy of Phi == j-blocked calls; ragged tiles."""
+    cfg = synth.Config("s", (20.52,) * 3, (32, 32, 32), 13, synth.KERNEL_HSE)
+    phi = synth.orbitals(cfg, device=cuda_device)
+    with binding.plan_for(cfg, block_i=4, block_j=4) as plan:
+        sym = plan.apply(phi)
+        assert plan.info()["last_symmetric"] == 1
+        gen = plan.apply(phi, phi.clone())
+        assert plan.info()["last_symmetric"] == 0
+        blk = torch.cat([plan.apply(phi, None, self_offset=o, n_targets=min(5, 13 - o)) for o in range(0, 13, 5)])
+        torch.cuda.synchronize()
+    ref = _oracle(cfg, phi)
+    for got in (sym, gen, blk):
+        assert _rel(got.cpu().numpy(), ref) <= TOL
+
+
+def test_host_path_and_stream(cuda_device):
+    cfg = synth.Config("h", (10.26,) * 3, (16, 16, 16), 6, synth.KERNEL_HSE, separate_psi=True)
+    phi, psi = synth.make_case(cfg, cuda_device)
+    with binding.plan_for(cfg) as plan:
+        ref = plan.apply(phi, psi)
+        host = plan.apply_host(phi.cpu().pin_memory(), psi.cpu().pin_memory())
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            on_s = plan.apply(phi, psi)
+        s.synchronize()
+        torch.cuda.synchronize()
+    assert torch.equal(host, ref.cpu()) and torch.equal(on_s, ref)
+
+
+def test_edge_cases_and_errors(cuda_device):
+    cfg = synth.Config("e", (10.26,) * 3, (16, 16, 16), 3, synth.KERNEL_HSE)
+    phi = synth.random_orbitals(cfg, 1, 3, cuda_device)
+    with binding.plan_for(cfg) as plan:
+        empty = plan.apply(phi, None, n_targets=0)
+        assert empty.shape[0] == 0
+        one = plan.apply(phi, None, self_offset=2, n_targets=1)
+        assert _rel(one.cpu().numpy(), _oracle(cfg, phi, cols=[2])) <= TOL
+        with pytest.raises(binding.PtfockError) as ei:
+            plan.apply(phi, None, out=phi)                       # alias
+        assert ei.value.code == -7
+        with pytest.raises(binding.PtfockError) as ei:
+            plan.apply(phi, None, self_offset=2, n_targets=2)    # out of range
+        assert ei.value.code == -1
+        mis = torch.empty(3 * cfg.N * 2 + 1, dtype=torch.float64, device=cuda_device)[1:].view(torch.complex128)
+        with pytest.raises(binding.PtfockError) as ei:
+            binding._check(binding.lib().ptfock_apply(plan._h, mis.data_ptr(), None, 0, 3, phi.data_ptr(), None), "x")
+        assert ei.value.code == -4
+    with pytest.raises(binding.PtfockError) as ei:
+        binding.Plan(cfg.cell, (16, 20, 16), 3)
+    assert ei.value.code == -2
+    with pytest.raises(binding.PtfockError) as ei:
+        binding.Plan(cfg.cell, (16, 16, 16), 3, kernel=5)
+    assert ei.value.code == -1
+    # single orbital, n_occ = 1
+    cfg1 = synth.Config("one", (10.26,) * 3, (16, 16, 16), 1, synth.KERNEL_COULOMB)
+    p1 = synth.random_orbitals(cfg1, 2, 1, cuda_device)
+    with binding.plan_for(cfg1) as plan:
+        o1 = plan.apply(p1)
+    assert _rel(o1.cpu().numpy(), _oracle(cfg1, p1)) <= TOL
