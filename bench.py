@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""Benchmark harness: Fock exchange pair-FFTs/s in fp64 on B200 (BASELINE.json ``metric``).
+
+One "step" = one whole pass of the hot path over one batch of synthetic input:
+  Si512  : ptfock_apply of 1024 targets against 1024 orbitals (1 048 576 pair-solves), 64^3 grid (default);
+  Si1536 : one streamed j-block of 96 targets against 3072 orbitals (294 912 pair-solves), 128x128x48;
+  Si8 / Si64 / Si216 : the full Psi = Phi application (pair-symmetric schedule).
+``value`` counts EFFECTIVE pair-solves N_i * N_j per second (equal to the executed count for Si512/Si1536).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config Si512] [--impl ours|reference]
+
+N > 1 (torchrun): the path is single-GPU by construction (BASELINE.json north_star), so ranks are independent
+replicas ("replicas only"); value = pairs of all ranks / max-over-ranks time.
+``--impl reference`` times the CPU oracle (oracle/ptfock_ref.c) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Fock exchange pair-FFTs/s (fp64, 1 B200) and % of HBM roofline"
+UNIT = "pair-FFTs/s"
+HBM_FALLBACK_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def load_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if r[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = [s for s, p in zip(sm, pw) if p >= 0.5 * max(pw)] or sm
+        return {"sm_mhz": statistics.median(busy), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload(cfg):
+    """(n_i, n_j, description) of one step."""
+    if cfg.j_block:
+        return cfg.n_occ, cfg.j_block, f"{cfg.name}: one j-block of {cfg.j_block} targets x {cfg.n_occ} orbitals"
+    return cfg.n_occ, cfg.n_occ, f"{cfg.name}: {cfg.n_occ} targets x {cfg.n_occ} orbitals"
+
+
+def cpu_sample(cfg, n_threads: int):
+    """Bounded oracle sample: (n_cols, n_i) sized for ~10-30 s of CPU work at this grid."""
+    rate_per_core = {4096: 1500.0, 32768: 170.0, 110592: 45.0, 262144: 17.0, 786432: 5.0}.get(cfg.N, 3e6 / cfg.N)
+    n_cols = min(n_threads, workload(cfg)[1])
+    n_i = int(max(1, min(cfg.n_occ, 15.0 * rate_per_core)))
+    return n_cols, n_i
+
+
+def run_oracle_sample(cfg, phi_np, psi_np, n_cols, n_i):
+    import numpy as np
+    import oracle
+    cols = list(range(n_cols))
+    phi_s = np.ascontiguousarray(phi_np[:n_i])
+    tgt = phi_np if psi_np is None else psi_np
+    tgt_s = np.ascontiguousarray(tgt[:n_cols])
+    t0 = time.perf_counter()
+    oracle.apply(cfg.cell, cfg.n, cfg.kernel, cfg.omega, cfg.alpha, phi_s, tgt_s, cols)
+    dt = time.perf_counter() - t0
+    return n_cols * n_i, dt
+
+
+def reference_arm(args, cfg):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    import torch
+    from paper_1905_01348_b200 import synth
+    oracle.build()
+    cores = oracle.num_threads()
+    n_cols, n_i = cpu_sample(cfg, cores)
+    n_orb = max(n_i, n_cols)
+    phi = synth.orbitals(cfg, cfg.seed_phi, n_orb, "cpu").numpy()
+    psi = synth.orbitals(cfg, cfg.seed_psi, n_cols, "cpu").numpy() if cfg.separate_psi else None
+    for _ in range(args.warmup):
+        run_oracle_sample(cfg, phi, psi, n_cols, min(n_i, 8))
+    pairs, secs = 0, 0.0
+    for _ in range(args.steps):
+        p, dt = run_oracle_sample(cfg, phi, psi, n_cols, n_i)
+        pairs += p
+        secs += dt
+    value = pairs / secs
+    sample = f"{n_cols} target columns x first {n_i} orbitals of {cfg.name} ({n_cols * n_i} pair-solves) per step"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload(cfg)[2], "grid": list(cfg.n), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="Si512")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--block-i", type=int, default=0)
+    ap.add_argument("--block-j", type=int, default=0)
+    ap.add_argument("--workspace-gb", type=float, default=0.0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")
+    args = ap.parse_args()
+
+    from paper_1905_01348_b200 import synth
+    cfg = synth.CONFIGS[args.config]
+    if args.impl == "reference":
+        reference_arm(args, cfg)
+        return
+
+    import torch
+    from paper_1905_01348_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    binding.lib()                                   # fails loudly if the CUDA library is missing
+    n_i, n_j, wl = workload(cfg)
+    phi = synth.orbitals(cfg, cfg.seed_phi, cfg.n_occ, dev)
+    psi = synth.orbitals(cfg, cfg.seed_psi, n_j, dev) if cfg.separate_psi else None
+    out = torch.empty((n_j,) + tuple(cfg.n), dtype=torch.complex128, device=dev)
+    plan = binding.plan_for(cfg, device=local, max_targets=n_j, block_i=args.block_i, block_j=args.block_j,
+                            workspace_bytes=int(args.workspace_gb * (1 << 30)))
+
+    def step():
+        if cfg.j_block:
+            plan.apply(phi, None, out=out, self_offset=0, n_targets=n_j)
+        else:
+            plan.apply(phi, psi, out=out)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    info0 = plan.info()
+    plan.set_profiling(True)
+    plan.get_profile(reset=True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    stream = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = e0.elapsed_time(e1)
+    prof = plan.get_profile(reset=True)
+    plan.set_profiling(False)
+    info1 = plan.info()
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    pairs_eff = n_i * n_j
+    pairs_exec = info1["last_pairs"]
+    value = world * pairs_eff / (ms_step * 1e-3)
+    launches = info1["total_launches"] - info0["total_launches"]
+
+    # ---- roofline of the dominant kernel (algorithmic bytes per launch / mean launch duration) -------
+    peak, peak_src = load_peak()
+    N = cfg.N
+    Ib, Jb = info1["block_i"], info1["block_j"]
+    names = ["slab_fwd (pass A)", "pencil_mid (pass B)", "slab_inv_acc (pass C)"]
+    # per executed pair-solve, in bytes: A reads its share of phi/psi and writes the pair density;
+    # B reads and writes it (v' table amortised over the wave); C reads it, reads phi_i, and
+    # read-modify-writes out once per (target, wave).
+    per_pair = [16.0 * N * (1.0 + 1.0 / Jb + 1.0 / Ib), 32.0 * N, 16.0 * N * (1.0 + 1.0 / Jb + 2.0 / Ib)]
+    shares = [m / max(1e-9, sum(prof["ms"])) for m in prof["ms"]]
+    k = max(range(3), key=lambda q: prof["ms"][q])
+    pairs_timed = pairs_exec * args.steps
+    achieved = [per_pair[q] * pairs_timed / max(1e-9, prof["ms"][q] * 1e-3) / 1e9 for q in range(3)]
+    roofline = {"bound": "hbm", "kernel": names[k], "achieved": achieved[k], "peak": peak, "unit": "GB/s",
+                "frac": achieved[k] / peak, "traffic": None, "peak_source": peak_src,
+                "bytes_per_pair_solve": per_pair[k], "launches": prof["launches"][k],
+                "avg_launch_ms": prof["ms"][k] / max(1, prof["launches"][k]),
+                "per_kernel": {names[q]: {"ms": prof["ms"][q], "share": shares[q], "GB/s": achieved[q],
+                                          "frac": achieved[q] / peak, "launches": prof["launches"][q]} for q in range(3)},
+                "path": {"bytes_per_pair_solve": sum(per_pair), "pairs_per_s_at_peak": peak * 1e9 / sum(per_pair),
+                         "frac": (pairs_exec / (ms_step * 1e-3)) / (peak * 1e9 / sum(per_pair)),
+                         "survey_72N_frac": (pairs_exec / (ms_step * 1e-3)) / (peak * 1e9 / (72.0 * N))}}
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            roofline["traffic"] = json.load(f).get(cfg.name, {}).get(names[k])
+    except Exception:
+        pass
+
+    # ---- end to end through the host-buffer entry point (pinned host memory, copies timed) -----------
+    e2e = None
+    if not args.no_e2e:
+        h_phi = torch.empty(phi.shape, dtype=phi.dtype, pin_memory=True).copy_(phi)
+        h_psi = torch.empty(psi.shape, dtype=psi.dtype, pin_memory=True).copy_(psi) if psi is not None else None
+        h_out = torch.empty(out.shape, dtype=out.dtype, pin_memory=True)
+        plan.apply_host(h_phi, h_psi, out=h_out, n_targets=n_j)                    # warm-up (allocates staging)
+        n_e2e = max(1, min(args.steps, 2))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            plan.apply_host(h_phi, h_psi, out=h_out, n_targets=n_j)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        gb = 16 * N
+        e2e = {"value": world * pairs_eff * n_e2e / dt, "unit": UNIT,
+               "h2d_bytes_per_step": gb * (cfg.n_occ + (n_j if psi is not None else 0)), "d2h_bytes_per_step": gb * n_j,
+               "steps": n_e2e, "api": "ptfock_apply_host (pinned host buffers)"}
+        del h_phi, h_psi
+
+    # ---- parity on sampled columns + CPU baseline (rank 0, N = 1 only) ------------------------------
+    cpu_baseline, parity = None, None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        import numpy as np
+        import oracle
+        oracle.build()
+        cores = oracle.num_threads()
+        n_cols, n_is = cpu_sample(cfg, cores)
+        phi_np = phi[:max(n_is, n_cols)].cpu().numpy()
+        psi_np = psi[:n_cols].cpu().numpy() if psi is not None else None
+        p, dt = run_oracle_sample(cfg, phi_np, psi_np, n_cols, n_is)
+        cpu_baseline = {"value": p / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"{n_cols} target columns x first {n_is} orbitals of {cfg.name} ({p} pair-solves, {dt:.1f} s)"}
+        if args.check:
+            cols = sorted({0, n_j // 2, n_j - 1})
+            tgt = phi if psi is None else psi
+            ref = oracle.apply(cfg.cell, cfg.n, cfg.kernel, cfg.omega, cfg.alpha, phi.cpu().numpy(),
+                               tgt[:n_j].cpu().numpy(), cols)
+            got = out[cols].cpu().numpy()
+            parity = {"columns": cols, "max_rel_err": float(np.abs(got - ref).max() / np.abs(ref).max())}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": wl, "grid": list(cfg.n), "n_i": n_i, "n_j": n_j,
+                           "kernel": "HSE" if cfg.kernel == 1 else "Coulomb",
+                           "pair_solves_executed_per_step": pairs_exec, "symmetric_schedule": bool(info1["last_symmetric"]),
+                           "block_i": Ib, "block_j": Jb, "scratch_bytes": info1["scratch_bytes"],
+                           "l2": f"inputs + scratch per step = {(16 * N * (n_i + 2 * n_j) + info1['scratch_bytes']) / 1e9:.2f} GB"
+                                 " (larger than the 126 MB L2; no explicit flush)",
+                           "parallelism": "replicas only" if world > 1 else "single GPU"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "cpu_baseline": cpu_baseline}
+        if parity:
+            line["parity"] = parity
+        print(json.dumps(line), flush=True)
+    plan.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

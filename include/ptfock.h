@@ -112,6 +112,13 @@ int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]);
  * v' = -alpha/N * v (so V_X psi_j = sum_i phi_i W_ij).  w_out: one grid, device.  Asynchronous. */
 int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const void *psi_j, void *w_out, void *stream);
 
+/* Per-pass device timing for the benchmark harness.  While on, every kernel launch of ptfock_apply is
+ * bracketed by cudaEvents on the caller's stream (pass 0 = slab forward "A", 1 = pencil middle "B",
+ * 2 = slab inverse + accumulate "C").  ptfock_get_profile waits for the last recorded event, returns the
+ * summed milliseconds and launch counts per pass since the last reset, and optionally resets. */
+int ptfock_set_profiling(ptfock_plan *plan, int32_t on);
+int ptfock_get_profile(ptfock_plan *plan, double ms[3], int64_t launches[3], int32_t reset);
+
 #ifdef __cplusplus
 }
 #endif

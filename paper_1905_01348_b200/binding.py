@@ -12,14 +12,15 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
-LIB_PATH = os.path.join(_HERE, "libptfock.so")
+LIB_PATH = os.environ.get("PTFOCK_LIB", os.path.join(_HERE, "libptfock.so"))
 SRC_DIR = os.path.join(_HERE, "csrc")
 
 KERNEL_COULOMB = 0
 KERNEL_HSE = 1
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
-           "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair"]
+           "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
+           "ptfock_set_profiling", "ptfock_get_profile"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -73,6 +74,8 @@ def lib() -> ctypes.CDLL:
         L.ptfock_last_cuda_error.argtypes = []
         L.ptfock_plan_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
         L.ptfock_debug_pair.argtypes = [vp, vp, vp, vp, vp]
+        L.ptfock_set_profiling.argtypes = [vp, i32]
+        L.ptfock_get_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64), i32]
         for name in EXPORTS:
             if name != "ptfock_strerror":
                 getattr(L, name).restype = ctypes.c_int
@@ -200,6 +203,15 @@ class Plan:
         _check(lib().ptfock_plan_info(self._h, a), "ptfock_plan_info")
         return {"block_i": a[0], "block_j": a[1], "scratch_bytes": a[2], "last_launches": a[3], "last_pairs": a[4],
                 "last_symmetric": a[5], "total_launches": a[6]}
+
+    def set_profiling(self, on: bool):
+        _check(lib().ptfock_set_profiling(self._h, 1 if on else 0), "ptfock_set_profiling")
+
+    def get_profile(self, reset: bool = True) -> dict:
+        ms = (ctypes.c_double * 3)()
+        cnt = (ctypes.c_int64 * 3)()
+        _check(lib().ptfock_get_profile(self._h, ms, cnt, 1 if reset else 0), "ptfock_get_profile")
+        return {"ms": [ms[0], ms[1], ms[2]], "launches": [cnt[0], cnt[1], cnt[2]]}
 
     def destroy(self):
         if self._h:

@@ -3,6 +3,7 @@
 // PAPER.md:149 "Batched implementation"; i <= j pair symmetry when Psi = Phi).
 #include "../../include/ptfock.h"
 #include "kernels.cuh"
+#include "slab2.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -45,6 +46,7 @@ struct SlabEntry {
     int n1, n2;
     slab_launch_fn fwd, inv;
     cudaError_t (*prepare)();
+    int ax1_r1, ax1_r2, ax2_r1, ax2_r2;     // digit split per axis: position k1*r2 + k2 holds frequency k1 + r1*k2
 };
 
 template <int N1, int N2> cudaError_t prepare_slab() {
@@ -55,12 +57,38 @@ template <int N1, int N2> cudaError_t prepare_slab() {
                                 SlabShape<N1, N2>::SMEM_BYTES);
 }
 
-#define SLAB(N1, N2) { N1, N2, launch_slab_fwd<N1, N2>, launch_slab_inv<N1, N2>, prepare_slab<N1, N2> }
+// register-resident 3-stage kernels (slab2.cuh)
+template <class S> void launch_slab2_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
+    slab2_fwd<S><<<grid, S::NT, S::SMEM_BYTES, st>>>(a);
+}
+template <class S> void launch_slab2_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) {
+    slab2_inv_acc<S><<<grid, S::NT, S::SMEM_BYTES, st>>>(a);
+}
+template <class S> cudaError_t prepare_slab2() {
+    cudaError_t e = cudaFuncSetAttribute(slab2_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(slab2_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES);
+}
+//            N1   N2  A1  B1  A2  B2  min CTAs/SM
+#ifndef PTF_MINB64
+#define PTF_MINB64 1
+#endif
+typedef Slab2<64, 64, 4, 16, 16, 4, PTF_MINB64> S2_64x64;
+typedef Slab2<128, 48, 8, 16, 16, 3, 1> S2_128x48;
+typedef Slab2<48, 48, 3, 16, 16, 3, 3> S2_48x48;
+typedef Slab2<32, 32, 2, 16, 16, 2, 8> S2_32x32;
+
+#define SLAB2(S) { S::N1, S::N2, launch_slab2_fwd<S>, launch_slab2_inv<S>, prepare_slab2<S>, S::A1, S::B1, S::A2, S::B2 }
+#define SLAB(N1, N2) { N1, N2, launch_slab_fwd<N1, N2>, launch_slab_inv<N1, N2>, prepare_slab<N1, N2>, \
+                       Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2 }
+// first match wins: the 3-stage kernels serve the BASELINE shapes, the generic 4-stage ones the rest
 const SlabEntry kSlabs[] = {
-    SLAB(16, 16), SLAB(32, 32), SLAB(48, 48), SLAB(64, 64), SLAB(128, 48),          // the five BASELINE configs
-    SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),           // non-square test shapes
+    SLAB2(S2_64x64), SLAB2(S2_128x48), SLAB2(S2_48x48), SLAB2(S2_32x32),
+    SLAB(16, 16), SLAB(32, 32), SLAB(48, 48), SLAB(64, 64), SLAB(128, 48),
+    SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),
 };
 #undef SLAB
+#undef SLAB2
 
 struct PencilEntry {
     int n0;
@@ -77,18 +105,18 @@ const PencilEntry kPencils[] = { PENCIL(16), PENCIL(32), PENCIL(48), PENCIL(64),
 #undef PENCIL
 
 // position -> frequency index of the digit-permuted order the forward passes leave an axis in
-int freq_of_pos(int n, int pos) {
-    int r1, r2;
-    switch (n) {
-        case 16: r1 = 16; r2 = 1; break;
-        case 32: r1 = 8; r2 = 4; break;
-        case 48: r1 = 16; r2 = 3; break;
-        case 64: r1 = 8; r2 = 8; break;
-        case 128: r1 = 16; r2 = 8; break;
-        default: return -1;
-    }
+int freq_of_pos(int r1, int r2, int pos) {
     const int k1 = pos / r2, k2 = pos % r2;
     return k1 + r1 * k2;
+}
+void pencil_split(int n, int &r1, int &r2) {
+    switch (n) {
+        case 16: r1 = Split<16>::R1; r2 = Split<16>::R2; break;
+        case 32: r1 = Split<32>::R1; r2 = Split<32>::R2; break;
+        case 48: r1 = Split<48>::R1; r2 = Split<48>::R2; break;
+        case 64: r1 = Split<64>::R1; r2 = Split<64>::R2; break;
+        default: r1 = Split<128>::R1; r2 = Split<128>::R2; break;
+    }
 }
 
 double det3(const double *a) {
@@ -123,6 +151,11 @@ struct ptfock_plan {
     // statistics
     long long last_launches, last_pairs, total_launches;
     int last_symmetric;
+    // optional per-pass device timing (ptfock_set_profiling): events bracket every launch
+    int profiling;
+    std::vector<cudaEvent_t> *ev_pool;
+    size_t ev_used;
+    std::vector<int> *ev_tags;         // tag of the interval that ENDS at event k (0/1/2 = pass A/B/C, -1 = none)
 };
 
 // ================================================================================================
@@ -148,12 +181,14 @@ void free_plan(ptfock_plan *p) {
     cudaFree(p->st_phi);
     cudaFree(p->st_psi);
     cudaFree(p->st_out);
+    if (p->ev_pool) { for (cudaEvent_t e : *p->ev_pool) cudaEventDestroy(e); delete p->ev_pool; }
+    delete p->ev_tags;
     delete p;
 }
 
 // v'(pos0, pos1, pos2) = -alpha/N * v(|G|^2) in the permuted order; also reports whether v(-G) = v(G)
 // holds on the grid (needed by the pair-symmetric schedule; fails for skew cells at Nyquist planes).
-int build_vtable(const ptfock_desc &d, std::vector<double> &vperm, bool &even) {
+int build_vtable(const ptfock_desc &d, const SlabEntry &se, std::vector<double> &vperm, bool &even) {
     const int n0 = d.n[0], n1 = d.n[1], n2 = d.n[2];
     const long long N = (long long)n0 * n1 * n2;
     const double *a = d.cell;
@@ -200,12 +235,14 @@ int build_vtable(const ptfock_desc &d, std::vector<double> &vperm, bool &even) {
             }
     const double scale = -d.alpha / (double)N;
     vperm.resize((size_t)N);
+    int p_r1, p_r2;
+    pencil_split(n0, p_r1, p_r2);
     for (int p0 = 0; p0 < n0; ++p0) {
-        const int k0 = freq_of_pos(n0, p0);
+        const int k0 = freq_of_pos(p_r1, p_r2, p0);
         for (int p1 = 0; p1 < n1; ++p1) {
-            const int k1 = freq_of_pos(n1, p1);
+            const int k1 = freq_of_pos(se.ax1_r1, se.ax1_r2, p1);
             for (int p2 = 0; p2 < n2; ++p2) {
-                const int k2 = freq_of_pos(n2, p2);
+                const int k2 = freq_of_pos(se.ax2_r1, se.ax2_r2, p2);
                 vperm[((size_t)p0 * n1 + p1) * n2 + p2] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
             }
         }
@@ -224,7 +261,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (!std::isfinite(d.alpha)) return PTFOCK_ERR_INVALID_ARG;
     for (int k = 0; k < 3; ++k) if (!edge_ok(d.n[k])) return PTFOCK_ERR_UNSUPPORTED_GRID;
     const SlabEntry *slab = nullptr;
-    for (const SlabEntry &e : kSlabs) if (e.n1 == d.n[1] && e.n2 == d.n[2]) slab = &e;
+    for (const SlabEntry &e : kSlabs) if (!slab && e.n1 == d.n[1] && e.n2 == d.n[2]) slab = &e;
     const PencilEntry *pencil = nullptr;
     for (const PencilEntry &e : kPencils) if (e.n0 == d.n[0]) pencil = &e;
     if (!slab || !pencil) return PTFOCK_ERR_UNSUPPORTED_GRID;
@@ -250,7 +287,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
 
     std::vector<double> vperm;
     bool even = false;
-    int rc = build_vtable(d, vperm, even);
+    int rc = build_vtable(d, *slab, vperm, even);
     if (rc != PTFOCK_OK) { free_plan(p); return rc; }
     p->v_even = even;
 
@@ -341,6 +378,22 @@ struct Wave {
     long long launches, pairs;
 };
 
+// profiling: record an event that closes an interval of kind `tag` (-1: opens a new run of intervals)
+void mark(Wave &w, int tag) {
+    ptfock_plan *p = w.p;
+    if (!p->profiling) return;
+    if (!p->ev_pool) { p->ev_pool = new std::vector<cudaEvent_t>(); p->ev_tags = new std::vector<int>(); }
+    if (p->ev_used == p->ev_pool->size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        p->ev_pool->push_back(e);
+        p->ev_tags->push_back(-1);
+    }
+    cudaEventRecord((*p->ev_pool)[p->ev_used], w.st);
+    (*p->ev_tags)[p->ev_used] = tag;
+    p->ev_used++;
+}
+
 // A + B for the block of pairs (i in [i0, i0+ni)) x (j in [j0, j0+nj)); pair index = ii * nj + jj.
 void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int j0, int nj) {
     ptfock_plan *p = w.p;
@@ -355,10 +408,13 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
     const long long base = (long long)p->d.n[0] * nj;
     while (z < ni && base * z < 148LL * 6) z *= 2;
     if (z > ni) z = ni;
+    mark(w, -1);
     p->slab->fwd(a, dim3(p->d.n[0], nj, z), w.st);
+    mark(w, 0);
     PencilArgs b;
     b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
     p->pencil->run(b, ni * nj, w.st);
+    mark(w, 1);
     w.launches += 2;
     w.pairs += (long long)ni * nj;
 }
@@ -374,6 +430,7 @@ void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, in
     a.a0 = s0; a.na = ns; a.b0 = t0;
     a.stride_loop = stride_loop; a.stride_cta = stride_cta; a.conj_w = conj_w;
     p->slab->inv(a, dim3(p->d.n[0], nt, 1), w.st);
+    mark(w, 2);
     w.launches += 1;
 }
 
@@ -521,5 +578,30 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(ones);
     if (e2 != cudaSuccess) { g_last_cuda = (int)e2; return PTFOCK_ERR_CUDA; }
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_set_profiling(ptfock_plan *plan, int32_t on) {
+    if (!plan) return PTFOCK_ERR_INVALID_ARG;
+    plan->profiling = on ? 1 : 0;
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_get_profile(ptfock_plan *plan, double ms[3], int64_t launches[3], int32_t reset) {
+    if (!plan || !ms || !launches) return PTFOCK_ERR_INVALID_ARG;
+    for (int k = 0; k < 3; ++k) { ms[k] = 0.0; launches[k] = 0; }
+    if (plan->ev_pool && plan->ev_used > 0) {
+        CU(cudaSetDevice(plan->d.device));
+        CU(cudaEventSynchronize((*plan->ev_pool)[plan->ev_used - 1]));
+        for (size_t k = 1; k < plan->ev_used; ++k) {
+            const int tag = (*plan->ev_tags)[k];
+            if (tag < 0) continue;
+            float t = 0.f;
+            CU(cudaEventElapsedTime(&t, (*plan->ev_pool)[k - 1], (*plan->ev_pool)[k]));
+            ms[tag] += (double)t;
+            launches[tag] += 1;
+        }
+    }
+    if (reset) plan->ev_used = 0;
     return PTFOCK_OK;
 }

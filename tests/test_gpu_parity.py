@@ -128,9 +128,9 @@ def test_edge_cases_and_errors(cuda_device):
         with pytest.raises(binding.PtfockError) as ei:
             plan.apply(phi, None, self_offset=2, n_targets=2)    # out of range
         assert ei.value.code == -1
-        mis = torch.empty(3 * cfg.N * 2 + 1, dtype=torch.float64, device=cuda_device)[1:].view(torch.complex128)
+        mis_ptr = phi.data_ptr() + 8
         with pytest.raises(binding.PtfockError) as ei:
-            binding._check(binding.lib().ptfock_apply(plan._h, mis.data_ptr(), None, 0, 3, phi.data_ptr(), None), "x")
+            binding._check(binding.lib().ptfock_apply(plan._h, mis_ptr, None, 0, 3, phi.data_ptr(), None), "x")
         assert ei.value.code == -4
     with pytest.raises(binding.PtfockError) as ei:
         binding.Plan(cfg.cell, (16, 20, 16), 3)
