@@ -161,6 +161,7 @@ def main():
     ap.add_argument("--block-i", type=int, default=0)
     ap.add_argument("--block-j", type=int, default=0)
     ap.add_argument("--workspace-gb", type=float, default=0.0)
+    ap.add_argument("--targets", type=int, default=0, help="restrict the step to the first T targets (profiling slices)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")
@@ -173,7 +174,7 @@ def main():
         return
 
     import torch
-    from paper_1905_01348_b200 import binding
+    from paper_1905_01348_b200 import binding, harness
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -188,12 +189,13 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
+        harness.barrier(dev)
 
     binding.lib()                                   # fails loudly if the CUDA library is missing
     n_i, n_j, wl = workload(cfg)
+    if args.targets:
+        n_j = min(n_j, args.targets)
+        wl += f" (slice: first {n_j} targets)"
     phi = synth.orbitals(cfg, cfg.seed_phi, cfg.n_occ, dev)
     psi = synth.orbitals(cfg, cfg.seed_psi, n_j, dev) if cfg.separate_psi else None
     out = torch.empty((n_j,) + tuple(cfg.n), dtype=torch.complex128, device=dev)
@@ -201,7 +203,7 @@ def main():
                             workspace_bytes=int(args.workspace_gb * (1 << 30)))
 
     def step():
-        if cfg.j_block:
+        if cfg.j_block or (args.targets and psi is None):
             plan.apply(phi, None, out=out, self_offset=0, n_targets=n_j)
         else:
             plan.apply(phi, psi, out=out)
@@ -228,10 +230,7 @@ def main():
     prof = plan.get_profile(reset=True)
     plan.set_profiling(False)
     info1 = plan.info()
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = harness.max_over_ranks(ms_total, dev)
     ms_step = ms_total / args.steps
     pairs_eff = n_i * n_j
     pairs_exec = info1["last_pairs"]
@@ -280,10 +279,7 @@ def main():
             plan.apply_host(h_phi, h_psi, out=h_out, n_targets=n_j)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = harness.max_over_ranks(dt, dev)
         gb = 16 * N
         e2e = {"value": world * pairs_eff * n_e2e / dt, "unit": UNIT,
                "h2d_bytes_per_step": gb * (cfg.n_occ + (n_j if psi is not None else 0)), "d2h_bytes_per_step": gb * n_j,

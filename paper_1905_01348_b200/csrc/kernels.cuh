@@ -121,7 +121,7 @@ struct SlabArgs {
 };
 
 // ---- pass A ---------------------------------------------------------------------------------------
-// grid = (n0, number of targets in the wave, chunks of the i loop); CTA (x0, jj, z) loops over its share of
+// grid = (number of targets in the wave, n0, chunks of the i loop); CTA (jj, x0, z) loops over its share of
 // the wave's orbitals i.
 template <int N1, int N2>
 __global__ void __launch_bounds__(kSlabThreads) slab_fwd(const SlabArgs g) {
@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(kSlabThreads) slab_fwd(const SlabArgs g) {
     const int tid = threadIdx.x;
     for (int t = tid; t < N1; t += kSlabThreads) tw1[t] = g.tw1[t];
     for (int t = tid; t < N2; t += kSlabThreads) tw2[t] = g.tw2[t];
-    const int x0 = blockIdx.x, jj = blockIdx.y;
+    const int x0 = blockIdx.y, jj = blockIdx.x;
     const long long slab_off = (long long)x0 * S::NPTS;
     const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + slab_off;
     cd pj[S::PER_THREAD];
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(kSlabThreads) slab_fwd(const SlabArgs g) {
 }
 
 // ---- pass C ---------------------------------------------------------------------------------------
-// grid = (n0, number of targets); CTA (x0, tt) sums over the looped orbitals s:
+// grid = (number of targets, n0); CTA (tt, x0) sums over the looped orbitals s:
 //   out[b0+tt] += sum_s a[a0+s] * W[s*stride_loop + tt*stride_cta]   (W or conj(W))
 template <int N1, int N2>
 __global__ void __launch_bounds__(kSlabThreads) slab_inv_acc(const SlabArgs g) {
@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(kSlabThreads) slab_inv_acc(const SlabArgs g) {
     const int tid = threadIdx.x;
     for (int t = tid; t < N1; t += kSlabThreads) tw1[t] = g.tw1[t];
     for (int t = tid; t < N2; t += kSlabThreads) tw2[t] = g.tw2[t];
-    const int x0 = blockIdx.x, tt = blockIdx.y;
+    const int x0 = blockIdx.y, tt = blockIdx.x;
     const long long slab_off = (long long)x0 * S::NPTS;
     cd acc[S::PER_THREAD];
 #pragma unroll

@@ -309,12 +309,12 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
         CUP(cudaMemcpy(p->tw_dev[k], tw.data(), sizeof(cd) * n, cudaMemcpyHostToDevice));
     }
     // pair-scheduler tile
-    int Ib = d.block_i > 0 ? d.block_i : 16;
+    int Ib = d.block_i > 0 ? d.block_i : 64;
     int Jb = d.block_j > 0 ? d.block_j : 8;
     if (Ib > d.n_occ) Ib = d.n_occ;
     if (Jb > d.max_targets) Jb = d.max_targets;
     const size_t pair_bytes = sizeof(cd) * (size_t)p->N;
-    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)2 << 30);
+    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)4 << 30);
     while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Jb > 1) Jb = (Jb + 1) / 2;
     if ((size_t)Ib * Jb * pair_bytes > limit) { free_plan(p); return PTFOCK_ERR_ALLOC; }
@@ -409,7 +409,7 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
     while (z < ni && base * z < 148LL * 6) z *= 2;
     if (z > ni) z = ni;
     mark(w, -1);
-    p->slab->fwd(a, dim3(p->d.n[0], nj, z), w.st);
+    p->slab->fwd(a, dim3(nj, p->d.n[0], z), w.st);
     mark(w, 0);
     PencilArgs b;
     b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
@@ -429,7 +429,7 @@ void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, in
     a.grid_pts = p->N; a.n0 = p->d.n[0];
     a.a0 = s0; a.na = ns; a.b0 = t0;
     a.stride_loop = stride_loop; a.stride_cta = stride_cta; a.conj_w = conj_w;
-    p->slab->inv(a, dim3(p->d.n[0], nt, 1), w.st);
+    p->slab->inv(a, dim3(nt, p->d.n[0], 1), w.st);
     mark(w, 2);
     w.launches += 1;
 }

@@ -78,6 +78,14 @@ PTF_DEV void stage2(cd *s, int t, const cd (&tw2r)[S::B2 > 1 ? S::B2 - 1 : 1], c
         for (int b2 = 0; b2 < B2; ++b2) p[a1 * B1 * P + b2] = u[a1][b2];
 }
 
+// Row handled by stage-1 thread group q (q = tid / B2).  Rows are dealt out so that the 8 lanes of a
+// quarter-warp hit 8 different 16-byte bank groups of the odd-pitch tile: bank = (x1 + b2) mod 8 = lane mod 8.
+template <class S>
+PTF_DEV int stage1_row(int q) {
+    if (S::N1 % S::B2 == 0) return S::B2 * (q % (S::N1 / S::B2)) + q / (S::N1 / S::B2);
+    return (S::B2 * q) % S::N1;        // gcd(B2, N1) = 1
+}
+
 template <class S>
 PTF_DEV void load_stage2_twiddles(const cd *tw1, const cd *tw2, int t, cd (&tw2r)[S::B2 > 1 ? S::B2 - 1 : 1],
                                   cd (&tw1r)[S::A1 > 1 ? S::A1 - 1 : 1]) {
@@ -95,11 +103,11 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slab2_fwd(const SlabArgs g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd *s = reinterpret_cast<cd *>(smem_raw);
     const int tid = threadIdx.x;
-    const int b2 = tid % B2, x1 = tid / B2;             // stage 1
+    const int b2 = tid % B2, x1 = stage1_row<S>(tid / B2);             // stage 1
     const int pos2 = tid % N2, k1a = tid / N2;          // stage 3
     cd tw2r[B2 > 1 ? B2 - 1 : 1], tw1r[A1 > 1 ? A1 - 1 : 1];
     load_stage2_twiddles<S>(g.tw1, g.tw2, tid < S::S2 ? tid : 0, tw2r, tw1r);
-    const int x0 = blockIdx.x, jj = blockIdx.y;
+    const int x0 = blockIdx.y, jj = blockIdx.x;     // CTAs that share the phi slabs run together (L2 reuse)
     const long long slab_off = (long long)x0 * S::NPTS;
     const int goff = x1 * N2 + b2;                        // + a2 * B2
     const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + slab_off + goff;
@@ -153,11 +161,11 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slab2_inv_acc(const SlabArgs g
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd *s = reinterpret_cast<cd *>(smem_raw);
     const int tid = threadIdx.x;
-    const int b2 = tid % B2, x1 = tid / B2;             // last stage (mirror of forward stage 1)
+    const int b2 = tid % B2, x1 = stage1_row<S>(tid / B2);             // last stage (mirror of forward stage 1)
     const int pos2 = tid % N2, k1a = tid / N2;          // first stage (mirror of forward stage 3)
     cd tw2r[B2 > 1 ? B2 - 1 : 1], tw1r[A1 > 1 ? A1 - 1 : 1];
     load_stage2_twiddles<S>(g.tw1, g.tw2, tid < S::S2 ? tid : 0, tw2r, tw1r);
-    const int x0 = blockIdx.x, tt = blockIdx.y;
+    const int x0 = blockIdx.y, tt = blockIdx.x;
     const long long slab_off = (long long)x0 * S::NPTS;
     const int goff = x1 * N2 + b2;
     cd acc[A2];
