@@ -92,11 +92,11 @@ template <bool INV> struct DFT<8, INV> {
 };
 
 template <bool INV> struct DFT<16, INV> {
-    static PTF_DEV void run(cd (&v)[16]) {
-        // 16 = 4 x 4: x = 4a + b.  DFT over a for each b, twiddle w16^(b k1), DFT over b for each k1,
-        // result index k1 + 4 k2.
+    // first half: 16 = 4 x 4, x = 4a + b.  DFT over a for each b, then the twiddles w16^(b k1).
+    // Afterwards v[4 k1 + b] = y[k1][b] and X[k1 + 4 k2] = DFT4 over b of y[k1][.].
+    static PTF_DEV void first_half(cd (&v)[16]) {
 #pragma unroll
-        for (int b = 0; b < 4; ++b) DFT<4, INV>::run(v[b], v[4 + b], v[8 + b], v[12 + b]);   // -> y[k1][b] at v[4 k1 + b]
+        for (int b = 0; b < 4; ++b) DFT<4, INV>::run(v[b], v[4 + b], v[8 + b], v[12 + b]);
         const cd w1 = make_double2(kCosPi8, -kSinPi8);        // w16^1 (forward sign)
         const cd w2 = make_double2(kSqrtHalf, -kSqrtHalf);    // w16^2
         const cd w3 = make_double2(kSinPi8, -kCosPi8);        // w16^3
@@ -111,8 +111,15 @@ template <bool INV> struct DFT<16, INV> {
         v[12 + 1] = twmul<INV>(v[12 + 1], w3);
         v[12 + 2] = twmul<INV>(v[12 + 2], w6);
         v[12 + 3] = twmul<INV>(v[12 + 3], w9);
+    }
+    // second half for one k1: on return v[4 k1 + k2] = X[k1 + 4 k2]
+    static PTF_DEV void second_half(cd (&v)[16], int k1) {
+        DFT<4, INV>::run(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);
+    }
+    static PTF_DEV void run(cd (&v)[16]) {
+        first_half(v);
 #pragma unroll
-        for (int k1 = 0; k1 < 4; ++k1) DFT<4, INV>::run(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);
+        for (int k1 = 0; k1 < 4; ++k1) second_half(v, k1);
         // v[4 k1 + k2] holds X[k1 + 4 k2]: transpose the 4x4 register tile (free: renaming)
 #pragma unroll
         for (int k1 = 0; k1 < 4; ++k1)
