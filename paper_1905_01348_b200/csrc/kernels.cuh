@@ -218,6 +218,7 @@ template <int N0> struct PencilShape {
     static constexpr int R1 = Split<N0>::R1, R2 = Split<N0>::R2;
     static constexpr int NT = (R2 == 1) ? 128 : 256;
     static constexpr int SMEM_BYTES = (R2 == 1) ? 0 : (N0 * CW + N0) * (int)sizeof(cd);
+    static constexpr int MINB = (N0 == 128) ? 2 : 1;       // 128: cap at 128 registers so two CTAs share an SM
 };
 
 struct PencilArgs {
@@ -228,7 +229,7 @@ struct PencilArgs {
 };
 
 template <int N0>
-__global__ void __launch_bounds__(PencilShape<N0>::NT) pencil_mid(const PencilArgs g) {
+__global__ void __launch_bounds__(PencilShape<N0>::NT, PencilShape<N0>::MINB) pencil_mid(const PencilArgs g) {
     using S = PencilShape<N0>;
     constexpr int R1 = S::R1, R2 = S::R2, CW = S::CW, NT = S::NT;
     const int tid = threadIdx.x;

@@ -5,6 +5,7 @@
 #include "kernels.cuh"
 #include "slab2.cuh"
 #include "slab3.cuh"
+#include "slabx.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -48,6 +49,9 @@ struct SlabEntry {
     slab_launch_fn fwd, inv;
     cudaError_t (*prepare)();
     int ax1_r1, ax1_r2, ax2_r1, ax2_r2;     // digit split per axis: position k1*r2 + k2 holds frequency k1 + r1*k2
+    int nt3;                                // 0: scratch slab is [pos1][pos2]; else slabx's free layout
+                                            //    s = m*nt3 + k2a*n1 + k1  (k1 natural), k2 = k2a + ax2_r1*m
+    int legacy;                             // 1: pre-slabx kernel (selected by PTFOCK_SLAB=legacy, for comparisons)
 };
 
 template <int N1, int N2> cudaError_t prepare_slab() {
@@ -94,6 +98,22 @@ template <class S> cudaError_t prepare_slab3() {
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(slab3_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, Slab3<S>::SMEM_BYTES_INV);
 }
+// TMA-fed in-place kernels (slabx.cuh)
+template <class S> void launch_slabx_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
+    slabx_fwd<S><<<grid, S::NT, S::SMEM_A, st>>>(a);
+}
+template <class S> void launch_slabx_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) {
+    slabx_inv_acc<S><<<grid, S::NT, S::SMEM_C, st>>>(a);
+}
+template <class S> cudaError_t prepare_slabx() {
+    cudaError_t e = cudaFuncSetAttribute(slabx_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_A);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(slabx_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_C);
+}
+//          N1   N2  A1  B1  A2  B2  kind Q
+typedef SX<64, 64, 16, 4, 4, 16, false> SX_64x64;
+typedef SX<128, 48, 8, 16, 3, 16, true> SX_128x48;
+#define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::NT3, 0 }
 //            N1   N2  A1  B1  A2  B2  min CTAs/SM
 #ifndef PTF_MINB64
 #define PTF_MINB64 1
@@ -103,19 +123,20 @@ typedef Slab2<128, 48, 8, 16, 16, 3, 1> S2_128x48;
 typedef Slab2<48, 48, 3, 16, 16, 3, 3> S2_48x48;
 typedef Slab2<32, 32, 2, 16, 16, 2, 8> S2_32x32;
 
-#define SLAB2P(S) { S::N1, S::N2, launch_slab2p_fwd<S>, launch_slab2p_inv<S>, prepare_slab2p<S>, S::A1, S::B1, S::A2, S::B2 }
+#define SLAB2P(S) { S::N1, S::N2, launch_slab2p_fwd<S>, launch_slab2p_inv<S>, prepare_slab2p<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
 // measured on B200 (64x64): the one-barrier pipeline wins for pass A, the three-barrier kernel for pass C
 template <class S> cudaError_t prepare_slab_mixed() {
     cudaError_t e = prepare_slab2p<S>();
     return e != cudaSuccess ? e : prepare_slab2<S>();
 }
-#define SLABMIX(S) { S::N1, S::N2, launch_slab2p_fwd<S>, launch_slab2_inv<S>, prepare_slab_mixed<S>, S::A1, S::B1, S::A2, S::B2 }
-#define SLAB3(S) { S::N1, S::N2, launch_slab3_fwd<S>, launch_slab3_inv<S>, prepare_slab3<S>, S::A1, S::B1, S::A2, S::B2 }
-#define SLAB2(S) { S::N1, S::N2, launch_slab2_fwd<S>, launch_slab2_inv<S>, prepare_slab2<S>, S::A1, S::B1, S::A2, S::B2 }
+#define SLABMIX(S) { S::N1, S::N2, launch_slab2p_fwd<S>, launch_slab2_inv<S>, prepare_slab_mixed<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
+#define SLAB3(S) { S::N1, S::N2, launch_slab3_fwd<S>, launch_slab3_inv<S>, prepare_slab3<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
+#define SLAB2(S) { S::N1, S::N2, launch_slab2_fwd<S>, launch_slab2_inv<S>, prepare_slab2<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
 #define SLAB(N1, N2) { N1, N2, launch_slab_fwd<N1, N2>, launch_slab_inv<N1, N2>, prepare_slab<N1, N2>, \
-                       Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2 }
+                       Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2, 0, 1 }
 // first match wins: the 3-stage kernels serve the BASELINE shapes, the generic 4-stage ones the rest
 const SlabEntry kSlabs[] = {
+    SLABX(SX_64x64), SLABX(SX_128x48),
 #ifdef PTF_USE_SLAB3
     SLAB3(S2_64x64),
 #endif
@@ -281,12 +302,17 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, std::vector<double> 
     pencil_split(n0, p_r1, p_r2);
     for (int p0 = 0; p0 < n0; ++p0) {
         const int k0 = freq_of_pos(p_r1, p_r2, p0);
-        for (int p1 = 0; p1 < n1; ++p1) {
-            const int k1 = freq_of_pos(se.ax1_r1, se.ax1_r2, p1);
-            for (int p2 = 0; p2 < n2; ++p2) {
-                const int k2 = freq_of_pos(se.ax2_r1, se.ax2_r2, p2);
-                vperm[((size_t)p0 * n1 + p1) * n2 + p2] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
+        for (int s = 0; s < n1 * n2; ++s) {
+            int k1, k2;
+            if (se.nt3) {
+                const int m = s / se.nt3, t = s % se.nt3;
+                k1 = t % n1;
+                k2 = (t / n1) + se.ax2_r1 * m;
+            } else {
+                k1 = freq_of_pos(se.ax1_r1, se.ax1_r2, s / n2);
+                k2 = freq_of_pos(se.ax2_r1, se.ax2_r2, s % n2);
             }
+            vperm[(size_t)p0 * n1 * n2 + s] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
         }
     }
     return PTFOCK_OK;
@@ -303,7 +329,10 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (!std::isfinite(d.alpha)) return PTFOCK_ERR_INVALID_ARG;
     for (int k = 0; k < 3; ++k) if (!edge_ok(d.n[k])) return PTFOCK_ERR_UNSUPPORTED_GRID;
     const SlabEntry *slab = nullptr;
-    for (const SlabEntry &e : kSlabs) if (!slab && e.n1 == d.n[1] && e.n2 == d.n[2]) slab = &e;
+    const char *pick = std::getenv("PTFOCK_SLAB");          // "legacy": the pre-slabx kernels (comparison runs only)
+    const bool legacy_only = pick && std::strcmp(pick, "legacy") == 0;
+    for (const SlabEntry &e : kSlabs)
+        if (!slab && e.n1 == d.n[1] && e.n2 == d.n[2] && (!legacy_only || e.legacy)) slab = &e;
     const PencilEntry *pencil = nullptr;
     for (const PencilEntry &e : kPencils) if (e.n0 == d.n[0]) pencil = &e;
     if (!slab || !pencil) return PTFOCK_ERR_UNSUPPORTED_GRID;

@@ -1,0 +1,413 @@
+// slabx.cuh -- TMA-fed, in-place slab passes (pass A and pass C of the BASELINE shapes 64x64 and 128x48).
+//
+// Same three butterfly stages per (x1, x2) slab as slab2.cuh, re-ordered so that every byte that crosses
+// the L1/shared-memory pipe is useful (ncu on the slab2 kernels: the LSU data pipe is the busiest unit,
+// and its orbital loads touched only half of every 128-byte line):
+//
+//   * x1 is transformed FIRST and x2 LAST.  Stage 1 threads own points that are consecutive in x2, so the
+//     psi_j / phi_i / out accesses of Eq. (3)'s products (Alg. 2 lines 7-9,
+//     PAPER.md:135-138) are full 128-byte lines.
+//   * The slab order inside the pair scratch is free (pass B only needs "same order as the v' table"):
+//     stage-3 thread t writes its m-th output at  m*NT3 + t, so scratch stores (pass A) and scratch loads
+//     (pass C) are perfectly coalesced as well.  Position s = m*NT3 + k2a*N1 + k1 holds the frequencies
+//     k1 (natural order) and k2 = k2a + A2*m.
+//   * phi_i slabs (pass A) and pair-density slabs (pass C) are brought in by 1-D bulk async copies (TMA,
+//     cp.async.bulk + mbarrier) straight into the padded tile the butterflies then work on IN PLACE, two
+//     or three tiles rotating; nothing is prefetched through registers, so 256 threads x <= 255 registers
+//     hold psi_j (pass A) or the sum over i (pass C) without spills, also for the 24-point stage of 128x48.
+//
+// Digit structure (decimation in frequency, mirrored in pass C):  x1 = a1*B1 + b1,  x2 = a2*B2 + b2
+//   kind P (64x64 : A1=16 B1=4 A2=4 B2=16):  S1 = DFT over a1 | S2 = 2-D DFT over (b1, a2) | S3 = DFT over b2
+//   kind Q (128x48: A1=8 B1=16 A2=3 B2=16):  S1 = 2-D DFT over (a1, a2) | S2 = DFT over b1  | S3 = DFT over b2
+// S1 has exactly 256 tasks (one per thread: psi_j / the accumulators live in its registers).
+#pragma once
+#include "kernels.cuh"
+#include "slab3.cuh"   // mbarrier / bulk-copy helpers
+
+namespace ptfock {
+
+template <int N1_, int N2_, int A1_, int B1_, int A2_, int B2_, bool Q_>
+struct SX {
+    static constexpr int N1 = N1_, N2 = N2_, A1 = A1_, B1 = B1_, A2 = A2_, B2 = B2_;
+    static constexpr bool Q = Q_;
+    static_assert(A1 * B1 == N1 && A2 * B2 == N2, "bad split");
+    static constexpr int NT = 256;
+    static constexpr int NPTS = N1 * N2;
+    static constexpr int R1 = A1, C1 = Q ? A2 : 1;          // stage-1 butterfly: R1 x C1 points
+    static constexpr int R2 = B1, C2 = Q ? 1 : A2;          // stage-2 butterfly
+    static constexpr int CB1 = Q ? B2 : N2;                 // stage-1 tasks: (b1, cb)
+    static constexpr int CB2 = Q ? N2 : B2;                 // stage-2 tasks: (k1a, cb)
+    static constexpr int NT1 = B1 * CB1, NT2 = A1 * CB2, NT3 = N1 * A2;
+    static_assert(NT1 == NT, "stage 1 must have one task per thread");
+        static constexpr int PM = NT3 + 1;                      // pass C tile: [m][k2a][row], odd pitch
+    static constexpr int TILE_A = A1 * (B1 * N2 + 1), TILE_C = B2 * PM;        // elements (Addr below)
+    static constexpr int MAXSM = 232448 - 64;
+    static constexpr int NBUF_A = (3 * TILE_A * 16 <= MAXSM) ? 3 : 2;
+    static constexpr int NBUF_C = (3 * TILE_C * 16 <= MAXSM) ? 3 : 2;
+    static constexpr int SMEM_A = NBUF_A * TILE_A * 16 + 64;
+    static constexpr int SMEM_C = NBUF_C * TILE_C * 16 + 64;
+    static constexpr int NTWR = (Q ? A1 : B1) > 1 ? (Q ? A1 : B1) - 1 : 1;
+    static constexpr int NTWC = A2 > 1 ? A2 - 1 : 1;
+};
+
+// u[r*C + c] <-> p[r*SR + c*SC]
+template <int R, int C, int SR, int SC>
+PTF_DEV void tile_load(cd (&u)[R * C], const cd *p) {
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int c = 0; c < C; ++c) u[r * C + c] = p[r * SR + c * SC];
+}
+template <int R, int C, int SR, int SC>
+PTF_DEV void tile_store(const cd (&u)[R * C], cd *p) {
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int c = 0; c < C; ++c) p[r * SR + c * SC] = u[r * C + c];
+}
+template <int R, int C, bool INV>
+PTF_DEV void dft_over_r(cd (&u)[R * C]) {
+    if constexpr (R > 1) {
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+            cd t[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) t[r] = u[r * C + c];
+            DFT<R, INV>::run(t);
+#pragma unroll
+            for (int r = 0; r < R; ++r) u[r * C + c] = t[r];
+        }
+    }
+}
+template <int R, int C, bool INV>
+PTF_DEV void dft_over_c(cd (&u)[R * C]) {
+    if constexpr (C > 1) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            cd t[C];
+#pragma unroll
+            for (int c = 0; c < C; ++c) t[c] = u[r * C + c];
+            DFT<C, INV>::run(t);
+#pragma unroll
+            for (int c = 0; c < C; ++c) u[r * C + c] = t[c];
+        }
+    }
+}
+template <int R, int C, bool CONJ>
+PTF_DEV void tw_rows(cd (&u)[R * C], const cd *tw) {        // u[r][.] *= tw[r-1]
+#pragma unroll
+    for (int r = 1; r < R; ++r)
+#pragma unroll
+        for (int c = 0; c < C; ++c) u[r * C + c] = CONJ ? cmulc(u[r * C + c], tw[r - 1]) : cmul(u[r * C + c], tw[r - 1]);
+}
+template <int R, int C, bool CONJ>
+PTF_DEV void tw_cols(cd (&u)[R * C], const cd *tw) {        // u[.][c] *= tw[c-1]
+#pragma unroll
+    for (int c = 1; c < C; ++c)
+#pragma unroll
+        for (int r = 0; r < R; ++r) u[r * C + c] = CONJ ? cmulc(u[r * C + c], tw[c - 1]) : cmul(u[r * C + c], tw[c - 1]);
+}
+
+// The twiddled stage (P: stage 2, Q: stage 1) of thread `t`:  twr = w_N1^(b1*k1a) (P: over b1, task k1a;
+// Q: over k1a, task b1), twc = w_N2^(b2*k2a) over k2a for the task's b2.
+template <class S>
+PTF_DEV void load_twiddles(const cd *tw1, const cd *tw2, int t, cd (&twr)[S::NTWR], cd (&twc)[S::NTWC]) {
+    const int cb = t % (S::Q ? S::CB1 : S::CB2), rb = t / (S::Q ? S::CB1 : S::CB2);   // Q: (b2, b1)   P: (b2, k1a)
+#pragma unroll
+    for (int q = 1; q <= (S::Q ? S::A1 : S::B1) - 1; ++q) twr[q - 1] = tw1[q * rb];
+#pragma unroll
+    for (int q = 1; q < S::A2; ++q) twc[q - 1] = tw2[q * cb];
+}
+
+// ---- tile addressing -------------------------------------------------------------------------------
+// A row is named by its digits (k1a, b1): row = k1a*B1 + b1.
+// pass A layout: A1 chunks of B1 dense rows, one element of padding per chunk (one bulk copy per chunk):
+//                (k1a, b1, col) -> k1a*CH + b1*N2 + col,  CH = B1*N2 + 1.
+// pass C layout: (k1a, b1, col) -> (col % B2)*PM + (col / B2)*N1 + (k1a + A1*b1)      [m][k2a][k1].
+template <class S, bool CL> struct Addr {
+    static constexpr int CH = S::B1 * S::N2 + 1;
+    static constexpr int RA = CL ? 1 : CH;                           // stride of +1 in k1a / a1 (row += B1)
+    static constexpr int RB = CL ? S::A1 : S::N2;                    // stride of +1 in b1 / k1b (row += 1)
+    static constexpr int COLB = CL ? S::N1 : S::B2;                  // stride of +B2 columns (next a2 / k2a)
+    static constexpr int COL1 = CL ? S::PM : 1;                      // stride of +1 column inside a B2 block
+    static PTF_DEV int at(int k1a, int b1, int col) {
+        return CL ? (col % S::B2) * S::PM + (col / S::B2) * S::N1 + k1a + S::A1 * b1 : k1a * CH + b1 * S::N2 + col;
+    }
+};
+
+template <class S, bool CL> PTF_DEV int s1_base(int t) {             // element (a1, a2) at base + a1*RA + a2*COLB
+    const int cb = t % S::CB1, b1 = t / S::CB1;
+    return Addr<S, CL>::at(0, b1, cb);
+}
+template <class S, bool CL> PTF_DEV int s2_base(int t) {             // element (b1, a2) at base + b1*RB + a2*COLB
+    const int cb = t % S::CB2, k1a = t / S::CB2;
+    return Addr<S, CL>::at(k1a, 0, cb);
+}
+// stage-3 task t = k2a*N1 + k1 with k1 = k1a + A1*k1b: consecutive lanes sit in different chunks of the pass A
+// tile (conflict-free), and k1 is the natural x1 frequency.
+template <class S, bool CL> PTF_DEV int s3_base(int t) {             // element b2 at base + b2*COL1
+    const int k1 = t % S::N1, k2a = t / S::N1;
+    return Addr<S, CL>::at(k1 % S::A1, k1 / S::A1, k2a * S::B2);
+}
+
+// ---- bulk-copy issue (warp 0) -------------------------------------------------------------------------
+PTF_DEV void l2_prefetch(const void *p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// pass A: A1 chunks of B1 rows -> padded chunks
+template <class S>
+PTF_DEV void issue_rows(cd *tile, const cd *src, unsigned long long *bar, int lane) {
+    if (lane == 0) mbar_expect_tx(bar, S::NPTS * 16u);
+    __syncwarp();
+    if (lane < S::A1) bulk_g2s(tile + lane * (S::B1 * S::N2 + 1), src + lane * (S::B1 * S::N2), S::B1 * S::N2 * 16u, bar);
+}
+// pass C: B2 blocks of NT3 elements -> padded blocks
+template <class S>
+PTF_DEV void issue_blocks(cd *tile, const cd *src, unsigned long long *bar, int lane) {
+    if (lane == 0) mbar_expect_tx(bar, S::NPTS * 16u);
+    __syncwarp();
+    if (lane < S::B2) bulk_g2s(tile + lane * S::PM, src + lane * S::NT3, S::NT3 * 16u, bar);
+}
+
+// ---- pass A ---------------------------------------------------------------------------------------
+// grid = (targets in the wave, n0, chunks of the i loop)
+template <class S>
+__global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
+    constexpr int N2 = S::N2, B1 = S::B1, B2 = S::B2, R1 = S::R1, C1 = S::C1, R2 = S::R2, C2 = S::C2;
+    constexpr int NT = S::NT, NBUF = S::NBUF_A, TILE = S::TILE_A;
+    using A = Addr<S, false>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cd *tiles = reinterpret_cast<cd *>(smem_raw);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * TILE * 16);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int x0 = blockIdx.y, jj = blockIdx.x;
+    const long long slab_off = (long long)x0 * S::NPTS;
+    const int per = (g.na + gridDim.z - 1) / gridDim.z;
+    const int ii_beg = blockIdx.z * per, ii_end = min(g.na, ii_beg + per);
+    const int n_it = ii_end - ii_beg;
+    if (n_it <= 0) return;
+    const cd *phi0 = g.a + (long long)(g.a0 + ii_beg) * g.grid_pts + slab_off;      // slab of the first orbital
+    if (tid == 0) {
+#pragma unroll
+        for (int b = 0; b < NBUF; ++b) mbar_init(&bars[b], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+    if (tid < 32) {
+        for (int it = 0; it < NBUF - 1 && it < n_it; ++it)
+            issue_rows<S>(tiles + it * TILE, phi0 + (long long)it * g.grid_pts, &bars[it], lane);
+    }
+    // stage-1 task of this thread: psi_j values in registers for the whole loop
+    const int cb = tid % S::CB1, b1 = tid / S::CB1;
+    const int base1 = s1_base<S, false>(tid);
+    cd pj[R1 * C1];
+    {
+        const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + slab_off + b1 * N2 + cb;
+        tile_load<R1, C1, B1 * N2, B2>(pj, psi);
+    }
+    cd twr[S::NTWR], twc[S::NTWC];
+    load_twiddles<S>(g.tw1, g.tw2, tid, twr, twc);
+    const int base2 = s2_base<S, false>(tid);            // P: the twiddled stage-2 task of this thread
+
+    for (int it = 0; it < n_it; ++it) {
+        const int b = it % NBUF;
+        cd *T = tiles + b * TILE;
+        mbar_wait(&bars[b], (it / NBUF) & 1);
+        {   // ---- stage 1: rho = psi_j conj(phi_i), DFT over a1 (Q: and a2, with both twiddles)
+            cd u[R1 * C1];
+            tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
+#pragma unroll
+            for (int k = 0; k < R1 * C1; ++k) u[k] = cmulc(pj[k], u[k]);
+            dft_over_r<R1, C1, false>(u);
+            if (S::Q) {
+                tw_rows<R1, C1, false>(u, twr);
+                dft_over_c<R1, C1, false>(u);
+                tw_cols<R1, C1, false>(u, twc);
+            }
+            tile_store<R1, C1, A::RA, A::COLB>(u, T + base1);
+        }
+        fence_proxy_async();
+        __syncthreads();
+        // the tile stage 3 of the previous orbital drained is refilled now
+        if (tid < 32 && it + NBUF - 1 < n_it) {
+            const int nx = it + NBUF - 1;
+            issue_rows<S>(tiles + (nx % NBUF) * TILE, phi0 + (long long)nx * g.grid_pts, &bars[nx % NBUF], lane);
+        }
+        // ---- stage 2
+        if (S::Q) {
+            for (int t = tid; t < S::NT2; t += NT) {
+                cd u[R2 * C2];
+                cd *p = T + s2_base<S, false>(t);
+                tile_load<R2, C2, A::RB, A::COLB>(u, p);
+                dft_over_r<R2, C2, false>(u);
+                tile_store<R2, C2, A::RB, A::COLB>(u, p);
+            }
+        } else {
+            cd u[R2 * C2];
+            tile_load<R2, C2, A::RB, A::COLB>(u, T + base2);
+            tw_rows<R2, C2, false>(u, twr);
+            dft_over_r<R2, C2, false>(u);
+            dft_over_c<R2, C2, false>(u);
+            tw_cols<R2, C2, false>(u, twc);
+            tile_store<R2, C2, A::RB, A::COLB>(u, T + base2);
+        }
+        __syncthreads();
+        // ---- stage 3: DFT over b2, straight to the pair scratch (free layout: m*NT3 + t)
+        cd *dst = g.scratch + ((long long)((ii_beg + it) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS;
+        for (int t = tid; t < S::NT3; t += NT) {
+            cd w[B2];
+            tile_load<1, B2, 0, A::COL1>(w, T + s3_base<S, false>(t));
+            DFT<B2, false>::run(w);
+#pragma unroll
+            for (int m = 0; m < B2; ++m) dst[m * S::NT3 + t] = w[m];
+        }
+    }
+}
+
+// ---- pass C ---------------------------------------------------------------------------------------
+// grid = (targets, n0): out[b0+tt] += sum_ss a[a0+ss] * W[ss*stride_loop + tt*stride_cta]   (W or conj(W))
+template <class S>
+__global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
+    constexpr int N2 = S::N2, B1 = S::B1, B2 = S::B2, R1 = S::R1, C1 = S::C1, R2 = S::R2, C2 = S::C2;
+    constexpr int NT = S::NT, NBUF = S::NBUF_C, TILE = S::TILE_C;
+    using A = Addr<S, true>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cd *tiles = reinterpret_cast<cd *>(smem_raw);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * TILE * 16);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int x0 = blockIdx.y, tt = blockIdx.x;
+    const long long slab_off = (long long)x0 * S::NPTS;
+    const int n_it = g.na;
+    if (n_it <= 0) return;
+    const long long pair_stride = (long long)g.stride_loop * g.n0 * S::NPTS;
+    const cd *src0 = g.scratch + ((long long)(tt * g.stride_cta) * g.n0 + x0) * S::NPTS;
+    if (tid == 0) {
+#pragma unroll
+        for (int b = 0; b < NBUF; ++b) mbar_init(&bars[b], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+    if (tid < 32) {
+        for (int it = 0; it < NBUF - 1 && it < n_it; ++it)
+            issue_blocks<S>(tiles + it * TILE, src0 + (long long)it * pair_stride, &bars[it], lane);
+    }
+    const int cb = tid % S::CB1, b1 = tid / S::CB1;
+    const int base1 = s1_base<S, true>(tid);
+    const cd *phi0 = g.a + (long long)g.a0 * g.grid_pts + slab_off + b1 * N2 + cb;
+    cd acc[R1 * C1];
+#pragma unroll
+    for (int k = 0; k < R1 * C1; ++k) acc[k] = make_double2(0.0, 0.0);
+    cd twr[S::NTWR], twc[S::NTWC];
+    load_twiddles<S>(g.tw1, g.tw2, tid, twr, twc);
+    const int base2 = s2_base<S, true>(tid);
+
+    for (int it = 0; it < n_it; ++it) {
+        const int b = it % NBUF;
+        cd *T = tiles + b * TILE;
+        const cd *phi = phi0 + (long long)it * g.grid_pts;
+        if (tid == 0 && it + 1 < n_it)      // next orbital's slab into L2 while this one is transformed
+            l2_prefetch(g.a + (long long)(g.a0 + it + 1) * g.grid_pts + slab_off, S::NPTS * 16u);
+        mbar_wait(&bars[b], (it / NBUF) & 1);
+        // ---- stage 1': inverse DFT over k2b (mirror of forward stage 3), in place
+        for (int t = tid; t < S::NT3; t += NT) {
+            cd w[B2];
+            cd *p = T + s3_base<S, true>(t);
+            tile_load<1, B2, 0, A::COL1>(w, p);
+            DFT<B2, true>::run(w);
+            tile_store<1, B2, 0, A::COL1>(w, p);
+        }
+        fence_proxy_async();
+        __syncthreads();
+        if (tid < 32 && it + NBUF - 1 < n_it) {
+            const int nx = it + NBUF - 1;
+            issue_blocks<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
+        }
+        if (!S::Q) {
+            // P: phi_i for the last stage, in flight during stage 2'
+            cd f[R1 * C1];
+            tile_load<R1, C1, B1 * N2, B2>(f, phi);
+            {
+                cd u[R2 * C2];
+                tile_load<R2, C2, A::RB, A::COLB>(u, T + base2);
+                tw_cols<R2, C2, true>(u, twc);
+                dft_over_c<R2, C2, true>(u);
+                dft_over_r<R2, C2, true>(u);
+                tw_rows<R2, C2, true>(u, twr);
+                tile_store<R2, C2, A::RB, A::COLB>(u, T + base2);
+            }
+            __syncthreads();
+            cd u[R1 * C1];
+            tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
+            dft_over_r<R1, C1, true>(u);
+            if (g.conj_w) {
+#pragma unroll
+                for (int k = 0; k < R1 * C1; ++k) {
+                    const cd pr = cmulc(f[k], u[k]);
+                    acc[k].x += pr.x; acc[k].y += pr.y;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < R1 * C1; ++k) {
+                    const cd pr = cmul(f[k], u[k]);
+                    acc[k].x += pr.x; acc[k].y += pr.y;
+                }
+            }
+        } else {
+            // Q: stage 2' = inverse DFT over k1b
+            for (int t = tid; t < S::NT2; t += NT) {
+                cd u[R2 * C2];
+                cd *p = T + s2_base<S, true>(t);
+                tile_load<R2, C2, A::RB, A::COLB>(u, p);
+                dft_over_r<R2, C2, true>(u);
+                tile_store<R2, C2, A::RB, A::COLB>(u, p);
+            }
+            __syncthreads();
+            // stage 3': 2-D inverse over (k1a, k2a); phi_i is fetched column block by column block
+            cd u[R1 * C1];
+            tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
+            cd f[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) f[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2));
+            tw_cols<R1, C1, true>(u, twc);
+            dft_over_c<R1, C1, true>(u);
+            tw_rows<R1, C1, true>(u, twr);
+#pragma unroll
+            for (int c = 0; c < C1; ++c) {
+                cd t[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) t[r] = u[r * C1 + c];
+                DFT<R1, true>::run(t);
+                cd fn[R1];
+                if (c + 1 < C1) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r)
+                        fn[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2 + (c + 1) * B2));
+                }
+#pragma unroll
+                for (int r = 0; r < R1; ++r) {
+                    const cd pr = g.conj_w ? cmulc(f[r], t[r]) : cmul(f[r], t[r]);
+                    acc[r * C1 + c].x += pr.x; acc[r * C1 + c].y += pr.y;
+                }
+                if (c + 1 < C1) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) f[r] = fn[r];
+                }
+            }
+        }
+    }
+    cd *o = g.out + (long long)(g.b0 + tt) * g.grid_pts + slab_off + b1 * N2 + cb;
+#pragma unroll
+    for (int r = 0; r < R1; ++r)
+#pragma unroll
+        for (int c = 0; c < C1; ++c) {
+            cd cur = o[r * B1 * N2 + c * B2];
+            cur.x += acc[r * C1 + c].x;
+            cur.y += acc[r * C1 + c].y;
+            o[r * B1 * N2 + c * B2] = cur;
+        }
+}
+
+}  // namespace ptfock
