@@ -211,6 +211,9 @@ __global__ void __launch_bounds__(kSlabThreads) slab_inv_acc(const SlabArgs g) {
     }
 }
 
+#ifndef PTF_PENCIL_MINB
+#define PTF_PENCIL_MINB 3
+#endif
 // ---- pass B ---------------------------------------------------------------------------------------
 // grid = (slab_pts / CW, pairs).  A CTA owns CW contiguous slab positions for all x0 of one pair.
 template <int N0> struct PencilShape {
@@ -218,7 +221,7 @@ template <int N0> struct PencilShape {
     static constexpr int R1 = Split<N0>::R1, R2 = Split<N0>::R2;
     static constexpr int NT = (R2 == 1) ? 128 : 256;
     static constexpr int SMEM_BYTES = (R2 == 1) ? 0 : (N0 * CW + N0) * (int)sizeof(cd);
-    static constexpr int MINB = (N0 == 128) ? 2 : 1;       // 128: cap at 128 registers so two CTAs share an SM
+    static constexpr int MINB = (N0 == 128) ? 2 : (R2 == 1 ? 1 : PTF_PENCIL_MINB);   // 128: two CTAs (128 regs) share an SM
 };
 
 struct PencilArgs {

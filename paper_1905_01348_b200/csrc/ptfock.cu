@@ -110,10 +110,13 @@ template <class S> cudaError_t prepare_slabx() {
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(slabx_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_C);
 }
-//          N1   N2  A1  B1  A2  B2  kind Q
-typedef SX<64, 64, 16, 4, 4, 16, false> SX_64x64;
-typedef SX<128, 48, 8, 16, 3, 16, true> SX_128x48;
-#define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::NT3, 0 }
+//          N1   N2  A1  B1  A2  B2  kind Q  bulk stores
+#ifndef PTF_TS64
+#define PTF_TS64 true
+#endif
+typedef SX<64, 64, 16, 4, 4, 16, false, PTF_TS64> SX_64x64;
+typedef SX<128, 48, 8, 16, 3, 16, true, false> SX_128x48;
+#define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3, 0 }
 //            N1   N2  A1  B1  A2  B2  min CTAs/SM
 #ifndef PTF_MINB64
 #define PTF_MINB64 1
@@ -381,7 +384,8 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     }
     // pair-scheduler tile
     int Ib = d.block_i > 0 ? d.block_i : 64;
-    int Jb = d.block_j > 0 ? d.block_j : 8;
+    // targets per wave: enough (target, x0) CTAs for ~7 full rounds of the 148 SMs in passes A and C
+    int Jb = d.block_j > 0 ? d.block_j : (1024 / d.n[0] > 8 ? 1024 / d.n[0] : 8);
     if (Ib > d.n_occ) Ib = d.n_occ;
     if (Jb > d.max_targets) Jb = d.max_targets;
     const size_t pair_bytes = sizeof(cd) * (size_t)p->N;

@@ -26,10 +26,13 @@
 
 namespace ptfock {
 
-template <int N1_, int N2_, int A1_, int B1_, int A2_, int B2_, bool Q_>
+// TS_: pass A hands its finished tile to bulk async STORES (the scratch slab is then the tile's own order,
+// [pos1][pos2], and pass C works in the pass A layout); otherwise stage 3 stores from registers in the free
+// layout above.  Needs three rotating tiles (the store has to drain before the tile is refilled).
+template <int N1_, int N2_, int A1_, int B1_, int A2_, int B2_, bool Q_, bool TS_>
 struct SX {
     static constexpr int N1 = N1_, N2 = N2_, A1 = A1_, B1 = B1_, A2 = A2_, B2 = B2_;
-    static constexpr bool Q = Q_;
+    static constexpr bool Q = Q_, TS = TS_, CLAYOUT = !TS_;
     static_assert(A1 * B1 == N1 && A2 * B2 == N2, "bad split");
     static constexpr int NT = 256;
     static constexpr int NPTS = N1 * N2;
@@ -39,13 +42,14 @@ struct SX {
     static constexpr int CB2 = Q ? N2 : B2;                 // stage-2 tasks: (k1a, cb)
     static constexpr int NT1 = B1 * CB1, NT2 = A1 * CB2, NT3 = N1 * A2;
     static_assert(NT1 == NT, "stage 1 must have one task per thread");
-        static constexpr int PM = NT3 + 1;                      // pass C tile: [m][k2a][row], odd pitch
-    static constexpr int TILE_A = A1 * (B1 * N2 + 1), TILE_C = B2 * PM;        // elements (Addr below)
+    static constexpr int PM = NT3 + 1;                      // pass C tile (free layout): [m][k2a][k1], odd pitch
+    static constexpr int TILE_A = A1 * (B1 * N2 + 1), TILE_C = TS ? TILE_A : B2 * PM;   // elements (Addr below)
     static constexpr int MAXSM = 232448 - 64;
     static constexpr int NBUF_A = (3 * TILE_A * 16 <= MAXSM) ? 3 : 2;
     static constexpr int NBUF_C = (3 * TILE_C * 16 <= MAXSM) ? 3 : 2;
     static constexpr int SMEM_A = NBUF_A * TILE_A * 16 + 64;
     static constexpr int SMEM_C = NBUF_C * TILE_C * 16 + 64;
+    static_assert(!TS || NBUF_A == 3, "bulk stores need three tiles");
     static constexpr int NTWR = (Q ? A1 : B1) > 1 ? (Q ? A1 : B1) - 1 : 1;
     static constexpr int NTWC = A2 > 1 ? A2 - 1 : 1;
 };
@@ -162,6 +166,20 @@ PTF_DEV void issue_rows(cd *tile, const cd *src, unsigned long long *bar, int la
     __syncwarp();
     if (lane < S::A1) bulk_g2s(tile + lane * (S::B1 * S::N2 + 1), src + lane * (S::B1 * S::N2), S::B1 * S::N2 * 16u, bar);
 }
+// pass A with bulk stores: padded chunks -> A1 chunks of B1 rows of the scratch slab (one bulk group per lane)
+PTF_DEV void bulk_s2g(void *dst_gmem, const void *src_smem, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes)
+                 : "memory");
+}
+PTF_DEV void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+PTF_DEV void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+template <class S>
+PTF_DEV void store_rows(const cd *tile, cd *dst, int lane) {
+    if (lane < S::A1) {
+        bulk_s2g(dst + lane * (S::B1 * S::N2), tile + lane * (S::B1 * S::N2 + 1), S::B1 * S::N2 * 16u);
+        bulk_commit();
+    }
+}
 // pass C: B2 blocks of NT3 elements -> padded blocks
 template <class S>
 PTF_DEV void issue_blocks(cd *tile, const cd *src, unsigned long long *bar, int lane) {
@@ -230,8 +248,13 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
         }
         fence_proxy_async();
         __syncthreads();
-        // the tile stage 3 of the previous orbital drained is refilled now
-        if (tid < 32 && it + NBUF - 1 < n_it) {
+        if (S::TS) {
+            // every thread has finished stage 3 of the previous orbital: its tile goes out as bulk stores
+            if (tid < 32 && it >= 1)
+                store_rows<S>(tiles + ((it - 1) % NBUF) * TILE,
+                              g.scratch + ((long long)((ii_beg + it - 1) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS, lane);
+        } else if (tid < 32 && it + NBUF - 1 < n_it) {
+            // the tile stage 3 of the previous orbital drained is refilled now
             const int nx = it + NBUF - 1;
             issue_rows<S>(tiles + (nx % NBUF) * TILE, phi0 + (long long)nx * g.grid_pts, &bars[nx % NBUF], lane);
         }
@@ -254,14 +277,41 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
             tile_store<R2, C2, A::RB, A::COLB>(u, T + base2);
         }
         __syncthreads();
-        // ---- stage 3: DFT over b2, straight to the pair scratch (free layout: m*NT3 + t)
-        cd *dst = g.scratch + ((long long)((ii_beg + it) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS;
-        for (int t = tid; t < S::NT3; t += NT) {
-            cd w[B2];
-            tile_load<1, B2, 0, A::COL1>(w, T + s3_base<S, false>(t));
-            DFT<B2, false>::run(w);
+        if (S::TS) {
+            // the previous tile's stores (issued one barrier ago by these lanes) have read it: refill it
+            if (tid < 32 && it + NBUF - 1 < n_it) {
+                const int nx = it + NBUF - 1;
+                bulk_wait_read_all();
+                __syncwarp();
+                issue_rows<S>(tiles + (nx % NBUF) * TILE, phi0 + (long long)nx * g.grid_pts, &bars[nx % NBUF], lane);
+            }
+            // ---- stage 3: DFT over b2, in place
+            for (int t = tid; t < S::NT3; t += NT) {
+                cd w[B2];
+                cd *p = T + s3_base<S, false>(t);
+                tile_load<1, B2, 0, A::COL1>(w, p);
+                DFT<B2, false>::run(w);
+                tile_store<1, B2, 0, A::COL1>(w, p);
+            }
+        } else {
+            // ---- stage 3: DFT over b2, straight to the pair scratch (free layout: m*NT3 + t)
+            cd *dst = g.scratch + ((long long)((ii_beg + it) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS;
+            for (int t = tid; t < S::NT3; t += NT) {
+                cd w[B2];
+                tile_load<1, B2, 0, A::COL1>(w, T + s3_base<S, false>(t));
+                DFT<B2, false>::run(w);
 #pragma unroll
-            for (int m = 0; m < B2; ++m) dst[m * S::NT3 + t] = w[m];
+                for (int m = 0; m < B2; ++m) dst[m * S::NT3 + t] = w[m];
+            }
+        }
+    }
+    if (S::TS) {
+        fence_proxy_async();
+        __syncthreads();
+        if (tid < 32) {
+            store_rows<S>(tiles + ((n_it - 1) % NBUF) * TILE,
+                          g.scratch + ((long long)((ii_end - 1) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS, lane);
+            bulk_wait_read_all();       // shared memory must outlive the reads
         }
     }
 }
@@ -272,7 +322,8 @@ template <class S>
 __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
     constexpr int N2 = S::N2, B1 = S::B1, B2 = S::B2, R1 = S::R1, C1 = S::C1, R2 = S::R2, C2 = S::C2;
     constexpr int NT = S::NT, NBUF = S::NBUF_C, TILE = S::TILE_C;
-    using A = Addr<S, true>;
+    constexpr bool CL = S::CLAYOUT;
+    using A = Addr<S, CL>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd *tiles = reinterpret_cast<cd *>(smem_raw);
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * TILE * 16);
@@ -292,17 +343,20 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
     __syncthreads();
     if (tid < 32) {
         for (int it = 0; it < NBUF - 1 && it < n_it; ++it)
-            issue_blocks<S>(tiles + it * TILE, src0 + (long long)it * pair_stride, &bars[it], lane);
+            {
+            if (CL) issue_blocks<S>(tiles + it * TILE, src0 + (long long)it * pair_stride, &bars[it], lane);
+            else issue_rows<S>(tiles + it * TILE, src0 + (long long)it * pair_stride, &bars[it], lane);
+        }
     }
     const int cb = tid % S::CB1, b1 = tid / S::CB1;
-    const int base1 = s1_base<S, true>(tid);
+    const int base1 = s1_base<S, CL>(tid);
     const cd *phi0 = g.a + (long long)g.a0 * g.grid_pts + slab_off + b1 * N2 + cb;
     cd acc[R1 * C1];
 #pragma unroll
     for (int k = 0; k < R1 * C1; ++k) acc[k] = make_double2(0.0, 0.0);
     cd twr[S::NTWR], twc[S::NTWC];
     load_twiddles<S>(g.tw1, g.tw2, tid, twr, twc);
-    const int base2 = s2_base<S, true>(tid);
+    const int base2 = s2_base<S, CL>(tid);
 
     for (int it = 0; it < n_it; ++it) {
         const int b = it % NBUF;
@@ -314,7 +368,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
         // ---- stage 1': inverse DFT over k2b (mirror of forward stage 3), in place
         for (int t = tid; t < S::NT3; t += NT) {
             cd w[B2];
-            cd *p = T + s3_base<S, true>(t);
+            cd *p = T + s3_base<S, CL>(t);
             tile_load<1, B2, 0, A::COL1>(w, p);
             DFT<B2, true>::run(w);
             tile_store<1, B2, 0, A::COL1>(w, p);
@@ -323,7 +377,8 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
         __syncthreads();
         if (tid < 32 && it + NBUF - 1 < n_it) {
             const int nx = it + NBUF - 1;
-            issue_blocks<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
+            if (CL) issue_blocks<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
+            else issue_rows<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
         }
         if (!S::Q) {
             // P: phi_i for the last stage, in flight during stage 2'
@@ -359,7 +414,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
             // Q: stage 2' = inverse DFT over k1b
             for (int t = tid; t < S::NT2; t += NT) {
                 cd u[R2 * C2];
-                cd *p = T + s2_base<S, true>(t);
+                cd *p = T + s2_base<S, CL>(t);
                 tile_load<R2, C2, A::RB, A::COLB>(u, p);
                 dft_over_r<R2, C2, true>(u);
                 tile_store<R2, C2, A::RB, A::COLB>(u, p);
