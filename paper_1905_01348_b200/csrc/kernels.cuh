@@ -217,11 +217,14 @@ __global__ void __launch_bounds__(kSlabThreads) slab_inv_acc(const SlabArgs g) {
 // ---- pass B ---------------------------------------------------------------------------------------
 // grid = (slab_pts / CW, pairs).  A CTA owns CW contiguous slab positions for all x0 of one pair.
 template <int N0> struct PencilShape {
-    static constexpr int CW = 32;
+#ifndef PTF_PENCIL128_CW
+#define PTF_PENCIL128_CW 16
+#endif
+    static constexpr int CW = (N0 == 128) ? PTF_PENCIL128_CW : 32;      // contiguous slab positions per CTA
     static constexpr int R1 = Split<N0>::R1, R2 = Split<N0>::R2;
-    static constexpr int NT = (R2 == 1) ? 128 : 256;
+    static constexpr int NT = (R2 == 1) ? 128 : CW * 8;
     static constexpr int SMEM_BYTES = (R2 == 1) ? 0 : (N0 * CW + N0) * (int)sizeof(cd);
-    static constexpr int MINB = (N0 == 128) ? 2 : (R2 == 1 ? 1 : PTF_PENCIL_MINB);   // 128: two CTAs (128 regs) share an SM
+    static constexpr int MINB = (N0 == 128) ? 64 / CW : (R2 == 1 ? 1 : PTF_PENCIL_MINB);   // 128: two CTAs (128 regs) share an SM
 };
 
 struct PencilArgs {

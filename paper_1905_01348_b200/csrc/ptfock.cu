@@ -115,7 +115,11 @@ template <class S> cudaError_t prepare_slabx() {
 #define PTF_TS64 true
 #endif
 typedef SX<64, 64, 16, 4, 4, 16, false, PTF_TS64> SX_64x64;
-typedef SX<128, 48, 8, 16, 3, 16, true, false> SX_128x48;
+#ifndef PTF_P128
+typedef SX<128, 48, 8, 16, 3, 16, true, false> SX_128x48;     // kind Q: 256 threads, 24-point first stage
+#else
+typedef SX<128, 48, 16, 8, 3, 16, false, false> SX_128x48;    // kind P: 384 threads, 24-point middle stage (spills: slower)
+#endif
 #define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3, 0 }
 //            N1   N2  A1  B1  A2  B2  min CTAs/SM
 #ifndef PTF_MINB64

@@ -34,22 +34,23 @@ struct SX {
     static constexpr int N1 = N1_, N2 = N2_, A1 = A1_, B1 = B1_, A2 = A2_, B2 = B2_;
     static constexpr bool Q = Q_, TS = TS_, CLAYOUT = !TS_;
     static_assert(A1 * B1 == N1 && A2 * B2 == N2, "bad split");
-    static constexpr int NT = 256;
     static constexpr int NPTS = N1 * N2;
     static constexpr int R1 = A1, C1 = Q ? A2 : 1;          // stage-1 butterfly: R1 x C1 points
     static constexpr int R2 = B1, C2 = Q ? 1 : A2;          // stage-2 butterfly
     static constexpr int CB1 = Q ? B2 : N2;                 // stage-1 tasks: (b1, cb)
     static constexpr int CB2 = Q ? N2 : B2;                 // stage-2 tasks: (k1a, cb)
     static constexpr int NT1 = B1 * CB1, NT2 = A1 * CB2, NT3 = N1 * A2;
-    static_assert(NT1 == NT, "stage 1 must have one task per thread");
+    static constexpr int NT = NT1;                          // stage 1 has one task per thread
+    static_assert(NT % 32 == 0 && NT <= 512 && (Q || NT2 <= NT), "bad thread count");
     static constexpr int PM = NT3 + 1;                      // pass C tile (free layout): [m][k2a][k1], odd pitch
     static constexpr int TILE_A = A1 * (B1 * N2 + 1), TILE_C = TS ? TILE_A : B2 * PM;   // elements (Addr below)
     static constexpr int MAXSM = 232448 - 64;
     static constexpr int NBUF_A = (3 * TILE_A * 16 <= MAXSM) ? 3 : 2;
     static constexpr int NBUF_C = (3 * TILE_C * 16 <= MAXSM) ? 3 : 2;
     static constexpr int SMEM_A = NBUF_A * TILE_A * 16 + 64;
-    static constexpr int SMEM_C = NBUF_C * TILE_C * 16 + 64;
+    static constexpr int SMEM_C = NBUF_C * TILE_C * 16 + 64 + (Q ? (N1 + N2) * 16 : 0);   // + twiddle tables (Q)
     static_assert(!TS || NBUF_A == 3, "bulk stores need three tiles");
+    static constexpr bool FUSE = NBUF_A == 3 && NBUF_C == 3;     // stage 3 of one orbital next to stage 1 of the next
     static constexpr int NTWR = (Q ? A1 : B1) > 1 ? (Q ? A1 : B1) - 1 : 1;
     static constexpr int NTWC = A2 > 1 ? A2 - 1 : 1;
 };
@@ -226,39 +227,24 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
         tile_load<R1, C1, B1 * N2, B2>(pj, psi);
     }
     cd twr[S::NTWR], twc[S::NTWC];
-    load_twiddles<S>(g.tw1, g.tw2, tid, twr, twc);
+    load_twiddles<S>(g.tw1, g.tw2, (S::Q || tid < S::NT2) ? tid : 0, twr, twc);
     const int base2 = s2_base<S, false>(tid);            // P: the twiddled stage-2 task of this thread
 
-    for (int it = 0; it < n_it; ++it) {
-        const int b = it % NBUF;
-        cd *T = tiles + b * TILE;
-        mbar_wait(&bars[b], (it / NBUF) & 1);
-        {   // ---- stage 1: rho = psi_j conj(phi_i), DFT over a1 (Q: and a2, with both twiddles)
-            cd u[R1 * C1];
-            tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
+    // ---- stage 1: rho = psi_j conj(phi_i), DFT over a1 (Q: and a2, with both twiddles), in place
+    auto stage1 = [&](cd *T) {
+        cd u[R1 * C1];
+        tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
 #pragma unroll
-            for (int k = 0; k < R1 * C1; ++k) u[k] = cmulc(pj[k], u[k]);
-            dft_over_r<R1, C1, false>(u);
-            if (S::Q) {
-                tw_rows<R1, C1, false>(u, twr);
-                dft_over_c<R1, C1, false>(u);
-                tw_cols<R1, C1, false>(u, twc);
-            }
-            tile_store<R1, C1, A::RA, A::COLB>(u, T + base1);
+        for (int k = 0; k < R1 * C1; ++k) u[k] = cmulc(pj[k], u[k]);
+        dft_over_r<R1, C1, false>(u);
+        if (S::Q) {
+            tw_rows<R1, C1, false>(u, twr);
+            dft_over_c<R1, C1, false>(u);
+            tw_cols<R1, C1, false>(u, twc);
         }
-        fence_proxy_async();
-        __syncthreads();
-        if (S::TS) {
-            // every thread has finished stage 3 of the previous orbital: its tile goes out as bulk stores
-            if (tid < 32 && it >= 1)
-                store_rows<S>(tiles + ((it - 1) % NBUF) * TILE,
-                              g.scratch + ((long long)((ii_beg + it - 1) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS, lane);
-        } else if (tid < 32 && it + NBUF - 1 < n_it) {
-            // the tile stage 3 of the previous orbital drained is refilled now
-            const int nx = it + NBUF - 1;
-            issue_rows<S>(tiles + (nx % NBUF) * TILE, phi0 + (long long)nx * g.grid_pts, &bars[nx % NBUF], lane);
-        }
-        // ---- stage 2
+        tile_store<R1, C1, A::RA, A::COLB>(u, T + base1);
+    };
+    auto stage2 = [&](cd *T) {
         if (S::Q) {
             for (int t = tid; t < S::NT2; t += NT) {
                 cd u[R2 * C2];
@@ -267,7 +253,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
                 dft_over_r<R2, C2, false>(u);
                 tile_store<R2, C2, A::RB, A::COLB>(u, p);
             }
-        } else {
+        } else if (S::NT2 == NT || tid < S::NT2) {
             cd u[R2 * C2];
             tile_load<R2, C2, A::RB, A::COLB>(u, T + base2);
             tw_rows<R2, C2, false>(u, twr);
@@ -276,33 +262,83 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
             tw_cols<R2, C2, false>(u, twc);
             tile_store<R2, C2, A::RB, A::COLB>(u, T + base2);
         }
-        __syncthreads();
-        if (S::TS) {
-            // the previous tile's stores (issued one barrier ago by these lanes) have read it: refill it
-            if (tid < 32 && it + NBUF - 1 < n_it) {
-                const int nx = it + NBUF - 1;
-                bulk_wait_read_all();
-                __syncwarp();
-                issue_rows<S>(tiles + (nx % NBUF) * TILE, phi0 + (long long)nx * g.grid_pts, &bars[nx % NBUF], lane);
-            }
-            // ---- stage 3: DFT over b2, in place
-            for (int t = tid; t < S::NT3; t += NT) {
-                cd w[B2];
-                cd *p = T + s3_base<S, false>(t);
-                tile_load<1, B2, 0, A::COL1>(w, p);
-                DFT<B2, false>::run(w);
+    };
+    // ---- stage 3: DFT over b2; TS: in place (the tile leaves by bulk stores), else registers -> scratch (m*NT3 + t)
+    auto stage3 = [&](cd *T, int it) {
+        cd *dst = g.scratch + ((long long)((ii_beg + it) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS;
+        for (int t = tid; t < S::NT3; t += NT) {
+            cd w[B2];
+            cd *p = T + s3_base<S, false>(t);
+            tile_load<1, B2, 0, A::COL1>(w, p);
+            DFT<B2, false>::run(w);
+            if (S::TS) {
                 tile_store<1, B2, 0, A::COL1>(w, p);
-            }
-        } else {
-            // ---- stage 3: DFT over b2, straight to the pair scratch (free layout: m*NT3 + t)
-            cd *dst = g.scratch + ((long long)((ii_beg + it) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS;
-            for (int t = tid; t < S::NT3; t += NT) {
-                cd w[B2];
-                tile_load<1, B2, 0, A::COL1>(w, T + s3_base<S, false>(t));
-                DFT<B2, false>::run(w);
+            } else {
 #pragma unroll
                 for (int m = 0; m < B2; ++m) dst[m * S::NT3 + t] = w[m];
             }
+        }
+    };
+    auto refill = [&](int nx) {     // warp 0: tile nx % NBUF <- phi slab of loop index nx
+        issue_rows<S>(tiles + (nx % NBUF) * TILE, phi0 + (long long)nx * g.grid_pts, &bars[nx % NBUF], lane);
+    };
+
+    mbar_wait(&bars[0], 0);
+    stage1(tiles);
+    for (int it = 0; it < n_it; ++it) {
+        cd *T = tiles + (it % NBUF) * TILE;
+        // here: stage 1 of orbital it and stage 3 of orbital it-1 are done by this thread
+        fence_proxy_async();
+        __syncthreads();
+        if (S::TS) {
+            if (tid < 32 && it >= 1)    // the previous orbital's finished tile goes out as bulk stores
+                store_rows<S>(tiles + ((it - 1) % NBUF) * TILE,
+                              g.scratch + ((long long)((ii_beg + it - 1) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS, lane);
+        } else if (tid < 32 && it + NBUF - 1 < n_it) {
+            refill(it + NBUF - 1);      // the tile stage 3 of the previous orbital drained
+        }
+        stage2(T);
+        __syncthreads();
+        if (S::TS && tid < 32 && it + NBUF - 1 < n_it) {
+            bulk_wait_read_all();       // the stores issued one barrier ago by these lanes have read their tile
+            __syncwarp();
+            refill(it + NBUF - 1);
+        }
+        if (it + 1 < n_it) {
+            cd *Tn = tiles + ((it + 1) % NBUF) * TILE;
+            if (S::FUSE) {
+                // the next tile landed long ago (three tiles): stage 3 of this orbital and stage 1 of the next one
+                // share a basic block, so one's shared-memory latency hides behind the other's arithmetic
+                mbar_wait(&bars[(it + 1) % NBUF], ((it + 1) / NBUF) & 1);
+                if (S::TS && S::NT3 == NT) {
+                    // both stages' shared-memory loads are issued before either stage's stores (the compiler
+                    // cannot prove the tiles distinct, so the order is spelled out here)
+                    cd w[B2], u[R1 * C1];
+                    cd *p3 = T + s3_base<S, false>(tid);
+                    tile_load<1, B2, 0, A::COL1>(w, p3);
+                    tile_load<R1, C1, A::RA, A::COLB>(u, Tn + base1);
+                    DFT<B2, false>::run(w);
+                    tile_store<1, B2, 0, A::COL1>(w, p3);
+#pragma unroll
+                    for (int k = 0; k < R1 * C1; ++k) u[k] = cmulc(pj[k], u[k]);
+                    dft_over_r<R1, C1, false>(u);
+                    if (S::Q) {
+                        tw_rows<R1, C1, false>(u, twr);
+                        dft_over_c<R1, C1, false>(u);
+                        tw_cols<R1, C1, false>(u, twc);
+                    }
+                    tile_store<R1, C1, A::RA, A::COLB>(u, Tn + base1);
+                } else {
+                    stage3(T, it);
+                    stage1(Tn);
+                }
+            } else {
+                stage3(T, it);
+                mbar_wait(&bars[(it + 1) % NBUF], ((it + 1) / NBUF) & 1);
+                stage1(Tn);
+            }
+        } else {
+            stage3(T, it);
         }
     }
     if (S::TS) {
@@ -354,18 +390,23 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
     cd acc[R1 * C1];
 #pragma unroll
     for (int k = 0; k < R1 * C1; ++k) acc[k] = make_double2(0.0, 0.0);
-    cd twr[S::NTWR], twc[S::NTWC];
-    load_twiddles<S>(g.tw1, g.tw2, tid, twr, twc);
+    // P: the twiddled stage's factors live in registers; Q (24-point last stage, 96 accumulator registers): they
+    // are re-read from a shared-memory copy of the two tables in every iteration instead
+    cd twr[S::Q ? 1 : S::NTWR], twc[S::Q ? 1 : S::NTWC];
+    cd *tws1 = reinterpret_cast<cd *>(smem_raw + (size_t)NBUF * TILE * 16 + 64), *tws2 = tws1 + S::N1;
+    if (S::Q) {
+        for (int t = tid; t < S::N1; t += NT) tws1[t] = g.tw1[t];
+        for (int t = tid; t < S::N2; t += NT) tws2[t] = g.tw2[t];
+        __syncthreads();
+    } else {
+        load_twiddles<S>(g.tw1, g.tw2, tid < S::NT2 ? tid : 0, *reinterpret_cast<cd (*)[S::NTWR]>(twr),
+                         *reinterpret_cast<cd (*)[S::NTWC]>(twc));
+    }
     const int base2 = s2_base<S, CL>(tid);
 
-    for (int it = 0; it < n_it; ++it) {
-        const int b = it % NBUF;
-        cd *T = tiles + b * TILE;
-        const cd *phi = phi0 + (long long)it * g.grid_pts;
-        if (tid == 0 && it + 1 < n_it)      // next orbital's slab into L2 while this one is transformed
-            l2_prefetch(g.a + (long long)(g.a0 + it + 1) * g.grid_pts + slab_off, S::NPTS * 16u);
-        mbar_wait(&bars[b], (it / NBUF) & 1);
-        // ---- stage 1': inverse DFT over k2b (mirror of forward stage 3), in place
+    // ---- stage 1': inverse DFT over k2b (mirror of forward stage 3), in place
+    auto stage1i = [&](cd *T) {
+#pragma unroll 1
         for (int t = tid; t < S::NT3; t += NT) {
             cd w[B2];
             cd *p = T + s3_base<S, CL>(t);
@@ -373,45 +414,10 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
             DFT<B2, true>::run(w);
             tile_store<1, B2, 0, A::COL1>(w, p);
         }
-        fence_proxy_async();
-        __syncthreads();
-        if (tid < 32 && it + NBUF - 1 < n_it) {
-            const int nx = it + NBUF - 1;
-            if (CL) issue_blocks<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
-            else issue_rows<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
-        }
-        if (!S::Q) {
-            // P: phi_i for the last stage, in flight during stage 2'
-            cd f[R1 * C1];
-            tile_load<R1, C1, B1 * N2, B2>(f, phi);
-            {
-                cd u[R2 * C2];
-                tile_load<R2, C2, A::RB, A::COLB>(u, T + base2);
-                tw_cols<R2, C2, true>(u, twc);
-                dft_over_c<R2, C2, true>(u);
-                dft_over_r<R2, C2, true>(u);
-                tw_rows<R2, C2, true>(u, twr);
-                tile_store<R2, C2, A::RB, A::COLB>(u, T + base2);
-            }
-            __syncthreads();
-            cd u[R1 * C1];
-            tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
-            dft_over_r<R1, C1, true>(u);
-            if (g.conj_w) {
-#pragma unroll
-                for (int k = 0; k < R1 * C1; ++k) {
-                    const cd pr = cmulc(f[k], u[k]);
-                    acc[k].x += pr.x; acc[k].y += pr.y;
-                }
-            } else {
-#pragma unroll
-                for (int k = 0; k < R1 * C1; ++k) {
-                    const cd pr = cmul(f[k], u[k]);
-                    acc[k].x += pr.x; acc[k].y += pr.y;
-                }
-            }
-        } else {
-            // Q: stage 2' = inverse DFT over k1b
+    };
+    auto stage2i = [&](cd *T) {
+        if (S::Q) {
+#pragma unroll 1
             for (int t = tid; t < S::NT2; t += NT) {
                 cd u[R2 * C2];
                 cd *p = T + s2_base<S, CL>(t);
@@ -419,37 +425,134 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
                 dft_over_r<R2, C2, true>(u);
                 tile_store<R2, C2, A::RB, A::COLB>(u, p);
             }
-            __syncthreads();
-            // stage 3': 2-D inverse over (k1a, k2a); phi_i is fetched column block by column block
-            cd u[R1 * C1];
-            tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
-            cd f[R1];
+        } else if (S::NT2 == NT || tid < S::NT2) {
+            cd u[R2 * C2];
+            tile_load<R2, C2, A::RB, A::COLB>(u, T + base2);
+            tw_cols<R2, C2, true>(u, twc);
+            dft_over_c<R2, C2, true>(u);
+            dft_over_r<R2, C2, true>(u);
+            tw_rows<R2, C2, true>(u, twr);
+            tile_store<R2, C2, A::RB, A::COLB>(u, T + base2);
+        }
+    };
+    // ---- stage 3' (P): inverse DFT over k1a, x phi_i (already in f), sum over i
+    auto stage3i_p = [&](cd *T, const cd (&f)[R1 * C1]) {
+        cd u[R1 * C1];
+        tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
+        dft_over_r<R1, C1, true>(u);
+        if (g.conj_w) {
 #pragma unroll
-            for (int r = 0; r < R1; ++r) f[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2));
-            tw_cols<R1, C1, true>(u, twc);
-            dft_over_c<R1, C1, true>(u);
-            tw_rows<R1, C1, true>(u, twr);
+            for (int k = 0; k < R1 * C1; ++k) {
+                const cd pr = cmulc(f[k], u[k]);
+                acc[k].x += pr.x; acc[k].y += pr.y;
+            }
+        } else {
 #pragma unroll
-            for (int c = 0; c < C1; ++c) {
-                cd t[R1];
+            for (int k = 0; k < R1 * C1; ++k) {
+                const cd pr = cmul(f[k], u[k]);
+                acc[k].x += pr.x; acc[k].y += pr.y;
+            }
+        }
+    };
+    // ---- stage 3' (Q): 2-D inverse over (k1a, k2a); phi_i is fetched column block by column block
+    auto stage3i_q = [&](cd *T, const cd *phi, cd (&f)[R1]) {
+        cd u[R1 * C1];
+        tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
 #pragma unroll
-                for (int r = 0; r < R1; ++r) t[r] = u[r * C1 + c];
-                DFT<R1, true>::run(t);
-                cd fn[R1];
-                if (c + 1 < C1) {
+        for (int c = 1; c < C1; ++c) {                         // conj(w_N2^(b2 k2a))
+            const cd w = tws2[c * cb];
 #pragma unroll
-                    for (int r = 0; r < R1; ++r)
-                        fn[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2 + (c + 1) * B2));
+            for (int r = 0; r < R1; ++r) u[r * C1 + c] = cmulc(u[r * C1 + c], w);
+        }
+        dft_over_c<R1, C1, true>(u);
+#pragma unroll
+        for (int r = 1; r < R1; ++r) {                         // conj(w_N1^(b1 k1a))
+            const cd w = tws1[r * b1];
+#pragma unroll
+            for (int c = 0; c < C1; ++c) u[r * C1 + c] = cmulc(u[r * C1 + c], w);
+        }
+#pragma unroll
+        for (int c = 0; c < C1; ++c) {
+            cd t[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) t[r] = u[r * C1 + c];
+            DFT<R1, true>::run(t);
+#pragma unroll
+            for (int r = 0; r < R1; ++r) {
+                const cd pr = g.conj_w ? cmulc(f[r], t[r]) : cmul(f[r], t[r]);
+                acc[r * C1 + c].x += pr.x; acc[r * C1 + c].y += pr.y;
+            }
+            if (c + 1 < C1) {
+#pragma unroll
+                for (int r = 0; r < R1; ++r)
+                    f[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2 + (c + 1) * B2));
+            }
+        }
+    };
+    auto refill = [&](int nx) {     // warp 0: tile nx % NBUF <- pair density of loop index nx
+        if (CL) issue_blocks<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
+        else issue_rows<S>(tiles + (nx % NBUF) * TILE, src0 + (long long)nx * pair_stride, &bars[nx % NBUF], lane);
+    };
+
+    mbar_wait(&bars[0], 0);
+    stage1i(tiles);
+    for (int it = 0; it < n_it; ++it) {
+        cd *T = tiles + (it % NBUF) * TILE;
+        const cd *phi = phi0 + (long long)it * g.grid_pts;
+        if (tid == 0 && it + 1 < n_it)      // next orbital's slab into L2 while this one is transformed
+            l2_prefetch(g.a + (long long)(g.a0 + it + 1) * g.grid_pts + slab_off, S::NPTS * 16u);
+        // here: stage 1' of pair it and stage 3' of pair it-1 are done by this thread
+        fence_proxy_async();
+        __syncthreads();
+        if (tid < 32 && it + NBUF - 1 < n_it) refill(it + NBUF - 1);
+        cd fq[S::Q ? R1 : 1];
+        if (S::Q) {     // first column block of phi_i: in flight during stage 2'
+#pragma unroll
+            for (int r = 0; r < R1; ++r) fq[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2));
+        }
+        stage2i(T);
+        __syncthreads();
+        const bool more = it + 1 < n_it;
+        cd *Tn = tiles + ((it + 1) % NBUF) * TILE;
+        if (!S::Q) {
+            if (more && S::FUSE && S::NT3 == NT) {
+                // stage 1' of the next pair and stage 3' of this one, loads first (see pass A)
+                mbar_wait(&bars[(it + 1) % NBUF], ((it + 1) / NBUF) & 1);
+                cd w[B2], u[R1 * C1], f[R1 * C1];
+                cd *p3 = Tn + s3_base<S, CL>(tid);
+                tile_load<1, B2, 0, A::COL1>(w, p3);
+                tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
+                DFT<B2, true>::run(w);
+                tile_store<1, B2, 0, A::COL1>(w, p3);
+                tile_load<R1, C1, B1 * N2, B2>(f, phi);      // phi_i (L2-prefetched): lands during the next DFT
+                dft_over_r<R1, C1, true>(u);
+                if (g.conj_w) {
+#pragma unroll
+                    for (int k = 0; k < R1 * C1; ++k) {
+                        const cd pr = cmulc(f[k], u[k]);
+                        acc[k].x += pr.x; acc[k].y += pr.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < R1 * C1; ++k) {
+                        const cd pr = cmul(f[k], u[k]);
+                        acc[k].x += pr.x; acc[k].y += pr.y;
+                    }
                 }
-#pragma unroll
-                for (int r = 0; r < R1; ++r) {
-                    const cd pr = g.conj_w ? cmulc(f[r], t[r]) : cmul(f[r], t[r]);
-                    acc[r * C1 + c].x += pr.x; acc[r * C1 + c].y += pr.y;
+            } else {
+                cd f[R1 * C1];
+                tile_load<R1, C1, B1 * N2, B2>(f, phi);
+                stage3i_p(T, f);
+                if (more) {
+                    mbar_wait(&bars[(it + 1) % NBUF], ((it + 1) / NBUF) & 1);
+                    stage1i(Tn);
                 }
-                if (c + 1 < C1) {
-#pragma unroll
-                    for (int r = 0; r < R1; ++r) f[r] = fn[r];
-                }
+            }
+        } else {
+            stage3i_q(T, phi, *reinterpret_cast<cd (*)[R1]>(fq));
+            if (more) {
+                mbar_wait(&bars[(it + 1) % NBUF], ((it + 1) / NBUF) & 1);
+                stage1i(Tn);
             }
         }
     }
