@@ -393,7 +393,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (Ib > d.n_occ) Ib = d.n_occ;
     if (Jb > d.max_targets) Jb = d.max_targets;
     const size_t pair_bytes = sizeof(cd) * (size_t)p->N;
-    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)4 << 30);
+    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)6 << 30);
     while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Jb > 1) Jb = (Jb + 1) / 2;
     if ((size_t)Ib * Jb * pair_bytes > limit) { free_plan(p); return PTFOCK_ERR_ALLOC; }
