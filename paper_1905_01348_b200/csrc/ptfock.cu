@@ -4,7 +4,6 @@
 #include "../../include/ptfock.h"
 #include "kernels.cuh"
 #include "slab2.cuh"
-#include "slab3.cuh"
 #include "slabx.cuh"
 
 #include <cmath>
@@ -74,30 +73,6 @@ template <class S> cudaError_t prepare_slab2() {
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(slab2_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES);
 }
-// pipelined 3-stage kernels: three rotating tiles, one barrier per orbital (slab2.cuh, second half)
-template <class S> void launch_slab2p_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
-    slab2p_fwd<S><<<grid, S::NT, Slab2P<S>::SMEM_BYTES, st>>>(a);
-}
-template <class S> void launch_slab2p_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) {
-    slab2p_inv_acc<S><<<grid, S::NT, Slab2P<S>::SMEM_BYTES, st>>>(a);
-}
-template <class S> cudaError_t prepare_slab2p() {
-    cudaError_t e = cudaFuncSetAttribute(slab2p_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, Slab2P<S>::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(slab2p_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, Slab2P<S>::SMEM_BYTES);
-}
-// warp-specialised 3-stage kernels (slab3.cuh)
-template <class S> void launch_slab3_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
-    slab3_fwd<S><<<grid, 2 * S::NT, Slab3<S>::SMEM_BYTES, st>>>(a);
-}
-template <class S> void launch_slab3_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) {
-    slab3_inv_acc<S><<<grid, 2 * S::NT, Slab3<S>::SMEM_BYTES_INV, st>>>(a);
-}
-template <class S> cudaError_t prepare_slab3() {
-    cudaError_t e = cudaFuncSetAttribute(slab3_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, Slab3<S>::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(slab3_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, Slab3<S>::SMEM_BYTES_INV);
-}
 // TMA-fed in-place kernels (slabx.cuh)
 template <class S> void launch_slabx_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
     slabx_fwd<S><<<grid, S::NT, S::SMEM_A, st>>>(a);
@@ -120,39 +95,21 @@ typedef SX<128, 48, 8, 16, 3, 16, true, false> SX_128x48;     // kind Q: 256 thr
 #else
 typedef SX<128, 48, 16, 8, 3, 16, false, false> SX_128x48;    // kind P: 384 threads, 24-point middle stage (spills: slower)
 #endif
+typedef SX<48, 48, 3, 16, 3, 16, true, false> SX_48x48;        // kind Q: 9-point first stage, 144-task DFT16 stages
+typedef SX<32, 32, 2, 16, 2, 16, true, false> SX_32x32;
 #define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3, 0 }
 //            N1   N2  A1  B1  A2  B2  min CTAs/SM
-#ifndef PTF_MINB64
-#define PTF_MINB64 1
-#endif
-typedef Slab2<64, 64, 4, 16, 16, 4, PTF_MINB64> S2_64x64;
+typedef Slab2<64, 64, 4, 16, 16, 4, 1> S2_64x64;
 typedef Slab2<128, 48, 8, 16, 16, 3, 1> S2_128x48;
 typedef Slab2<48, 48, 3, 16, 16, 3, 3> S2_48x48;
 typedef Slab2<32, 32, 2, 16, 16, 2, 8> S2_32x32;
 
-#define SLAB2P(S) { S::N1, S::N2, launch_slab2p_fwd<S>, launch_slab2p_inv<S>, prepare_slab2p<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
-// measured on B200 (64x64): the one-barrier pipeline wins for pass A, the three-barrier kernel for pass C
-template <class S> cudaError_t prepare_slab_mixed() {
-    cudaError_t e = prepare_slab2p<S>();
-    return e != cudaSuccess ? e : prepare_slab2<S>();
-}
-#define SLABMIX(S) { S::N1, S::N2, launch_slab2p_fwd<S>, launch_slab2_inv<S>, prepare_slab_mixed<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
-#define SLAB3(S) { S::N1, S::N2, launch_slab3_fwd<S>, launch_slab3_inv<S>, prepare_slab3<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
 #define SLAB2(S) { S::N1, S::N2, launch_slab2_fwd<S>, launch_slab2_inv<S>, prepare_slab2<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
 #define SLAB(N1, N2) { N1, N2, launch_slab_fwd<N1, N2>, launch_slab_inv<N1, N2>, prepare_slab<N1, N2>, \
                        Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2, 0, 1 }
 // first match wins: the 3-stage kernels serve the BASELINE shapes, the generic 4-stage ones the rest
 const SlabEntry kSlabs[] = {
-    SLABX(SX_64x64), SLABX(SX_128x48),
-#ifdef PTF_USE_SLAB3
-    SLAB3(S2_64x64),
-#endif
-#ifdef PTF_USE_SLAB2P
-    SLAB2P(S2_64x64),
-#endif
-#ifndef PTF_NO_SLABMIX
-    SLABMIX(S2_64x64),
-#endif
+    SLABX(SX_64x64), SLABX(SX_128x48), SLABX(SX_48x48), SLABX(SX_32x32),
     SLAB2(S2_64x64), SLAB2(S2_128x48), SLAB2(S2_48x48), SLAB2(S2_32x32),
     SLAB(16, 16), SLAB(32, 32), SLAB(48, 48), SLAB(64, 64), SLAB(128, 48),
     SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),

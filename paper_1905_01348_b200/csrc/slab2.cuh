@@ -231,156 +231,3 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slab2_inv_acc(const SlabArgs g
 }
 
 }  // namespace ptfock
-
-// =====================================================================================================
-// Pipelined variants: three rotating tiles, ONE CTA barrier per orbital.  In each barrier interval a warp
-// runs stage 3 of orbital it-2, stage 2 of orbital it-1 and stage 1 of orbital it back to back, so warps are
-// free to drift apart inside the interval and the shared-memory/L1 pipe of one warp overlaps the FP64 pipe of
-// another (ncu on the 3-barrier version: L1 pipe ~60 % busy, FP64 ~35 % busy, taking turns).
-// =====================================================================================================
-namespace ptfock {
-
-template <class S> struct Slab2P {
-    static constexpr int TILE = S::N1 * S::P;
-    static constexpr int SMEM_BYTES = 3 * TILE * (int)sizeof(cd);
-    static_assert(S::S2 <= S::NT, "stage 2 must fit the CTA");
-};
-
-template <class S>
-__global__ void __launch_bounds__(S::NT, 1) slab2p_fwd(const SlabArgs g) {
-    constexpr int N2 = S::N2, A1 = S::A1, B1 = S::B1, A2 = S::A2, B2 = S::B2, P = S::P;
-    constexpr int TILE = Slab2P<S>::TILE;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cd *tiles = reinterpret_cast<cd *>(smem_raw);
-    const int tid = threadIdx.x;
-    const int b2 = tid % B2, x1 = stage1_row<S>(tid / B2);
-    const int pos2 = tid % N2, k1a = tid / N2;
-    cd tw2r[B2 > 1 ? B2 - 1 : 1], tw1r[A1 > 1 ? A1 - 1 : 1];
-    load_stage2_twiddles<S>(g.tw1, g.tw2, tid < S::S2 ? tid : 0, tw2r, tw1r);
-    const int x0 = blockIdx.y, jj = blockIdx.x;
-    const long long slab_off = (long long)x0 * S::NPTS;
-    const int goff = x1 * N2 + b2;
-    const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + slab_off + goff;
-    cd pj[A2];
-#pragma unroll
-    for (int a2 = 0; a2 < A2; ++a2) pj[a2] = psi[a2 * B2];
-    const int per = (g.na + gridDim.z - 1) / gridDim.z;
-    const int ii_beg = blockIdx.z * per, ii_end = min(g.na, ii_beg + per);
-    const int n_it = ii_end - ii_beg;
-    if (n_it <= 0) return;
-    const cd *phi0 = g.a + (long long)(g.a0 + ii_beg) * g.grid_pts + slab_off + goff;
-    cd v[A2];
-#pragma unroll
-    for (int a2 = 0; a2 < A2; ++a2) v[a2] = __ldg(reinterpret_cast<const double2 *>(phi0 + a2 * B2));
-    int t1 = 0, t2 = 2, t3 = 1;                       // tile index of stage 1 / 2 / 3 work in this interval
-    for (int it = 0; it < n_it + 2; ++it) {
-        if (it >= 2) {                                 // stage 3 of orbital it-2
-            const cd *s = tiles + t3 * TILE;
-            cd w[B1];
-#pragma unroll
-            for (int q = 0; q < B1; ++q) w[q] = s[(k1a * B1 + q) * P + pos2];
-            DFT<B1, false>::run(w);
-            cd *dst = g.scratch + ((long long)((ii_beg + it - 2) * g.stride_loop + jj * g.stride_cta) * g.n0 + x0) * S::NPTS +
-                      k1a * B1 * N2 + pos2;
-#pragma unroll
-            for (int q = 0; q < B1; ++q) dst[q * N2] = w[q];
-        }
-        if (it >= 1 && it - 1 < n_it) {               // stage 2 of orbital it-1
-            if (tid < S::S2) stage2<S, false>(tiles + t2 * TILE, tid, tw2r, tw1r);
-        }
-        if (it < n_it) {                               // stage 1 of orbital it, then prefetch orbital it+1
-            cd *d = tiles + t1 * TILE + x1 * P + b2;
-#pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) v[a2] = cmulc(pj[a2], v[a2]);
-            DFT<A2, false>::run(v);
-#pragma unroll
-            for (int k = 0; k < A2; ++k) d[k * B2] = v[k];
-            if (it + 1 < n_it) {
-                const cd *phi = phi0 + (long long)(it + 1) * g.grid_pts;
-#pragma unroll
-                for (int a2 = 0; a2 < A2; ++a2) v[a2] = __ldg(reinterpret_cast<const double2 *>(phi + a2 * B2));
-            }
-        }
-        __syncthreads();
-        const int t = t3; t3 = t2; t2 = t1; t1 = t;   // rotate: the tile stage 3 just drained is refilled next
-    }
-}
-
-template <class S>
-__global__ void __launch_bounds__(S::NT, 1) slab2p_inv_acc(const SlabArgs g) {
-    constexpr int N2 = S::N2, A1 = S::A1, B1 = S::B1, A2 = S::A2, B2 = S::B2, P = S::P;
-    constexpr int TILE = Slab2P<S>::TILE;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cd *tiles = reinterpret_cast<cd *>(smem_raw);
-    const int tid = threadIdx.x;
-    const int b2 = tid % B2, x1 = stage1_row<S>(tid / B2);
-    const int pos2 = tid % N2, k1a = tid / N2;
-    cd tw2r[B2 > 1 ? B2 - 1 : 1], tw1r[A1 > 1 ? A1 - 1 : 1];
-    load_stage2_twiddles<S>(g.tw1, g.tw2, tid < S::S2 ? tid : 0, tw2r, tw1r);
-    const int x0 = blockIdx.y, tt = blockIdx.x;
-    const long long slab_off = (long long)x0 * S::NPTS;
-    const int goff = x1 * N2 + b2;
-    const int n_it = g.na;
-    if (n_it <= 0) return;
-    cd acc[A2];
-#pragma unroll
-    for (int a2 = 0; a2 < A2; ++a2) acc[a2] = make_double2(0.0, 0.0);
-    const long long pair_stride = (long long)g.stride_loop * g.n0 * S::NPTS;
-    const cd *src0 = g.scratch + ((long long)(tt * g.stride_cta) * g.n0 + x0) * S::NPTS + k1a * B1 * N2 + pos2;
-    const cd *phi0 = g.a + (long long)g.a0 * g.grid_pts + slab_off + goff;
-    cd w[B1];
-#pragma unroll
-    for (int q = 0; q < B1; ++q) w[q] = src0[q * N2];
-    int t1 = 0, t2 = 2, t3 = 1;
-    for (int it = 0; it < n_it + 2; ++it) {
-        if (it >= 2) {                                 // stage 3' of orbital it-2: x phi, accumulate
-            const cd *s = tiles + t3 * TILE + x1 * P + b2;
-            const cd *phi = phi0 + (long long)(it - 2) * g.grid_pts;
-            cd f[A2], v[A2];
-#pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) f[a2] = __ldg(reinterpret_cast<const double2 *>(phi + a2 * B2));
-#pragma unroll
-            for (int k = 0; k < A2; ++k) v[k] = s[k * B2];
-            DFT<A2, true>::run(v);
-            if (g.conj_w) {
-#pragma unroll
-                for (int a2 = 0; a2 < A2; ++a2) {
-                    const cd pr = cmulc(f[a2], v[a2]);
-                    acc[a2].x += pr.x; acc[a2].y += pr.y;
-                }
-            } else {
-#pragma unroll
-                for (int a2 = 0; a2 < A2; ++a2) {
-                    const cd pr = cmul(f[a2], v[a2]);
-                    acc[a2].x += pr.x; acc[a2].y += pr.y;
-                }
-            }
-        }
-        if (it >= 1 && it - 1 < n_it) {               // stage 2' of orbital it-1
-            if (tid < S::S2) stage2<S, true>(tiles + t2 * TILE, tid, tw2r, tw1r);
-        }
-        if (it < n_it) {                               // stage 1' of orbital it, then prefetch the next pair density
-            cd *s = tiles + t1 * TILE;
-            DFT<B1, true>::run(w);
-#pragma unroll
-            for (int q = 0; q < B1; ++q) s[(k1a * B1 + q) * P + pos2] = w[q];
-            if (it + 1 < n_it) {
-                const cd *src = src0 + (long long)(it + 1) * pair_stride;
-#pragma unroll
-                for (int q = 0; q < B1; ++q) w[q] = src[q * N2];
-            }
-        }
-        __syncthreads();
-        const int t = t3; t3 = t2; t2 = t1; t1 = t;
-    }
-    cd *o = g.out + (long long)(g.b0 + tt) * g.grid_pts + slab_off + goff;
-#pragma unroll
-    for (int a2 = 0; a2 < A2; ++a2) {
-        cd cur = o[a2 * B2];
-        cur.x += acc[a2].x;
-        cur.y += acc[a2].y;
-        o[a2 * B2] = cur;
-    }
-}
-
-}  // namespace ptfock

@@ -22,7 +22,7 @@
 // S1 has exactly 256 tasks (one per thread: psi_j / the accumulators live in its registers).
 #pragma once
 #include "kernels.cuh"
-#include "slab3.cuh"   // mbarrier / bulk-copy helpers
+#include "tma.cuh"
 
 namespace ptfock {
 

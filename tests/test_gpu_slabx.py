@@ -1,5 +1,5 @@
 """GPU vs oracle parity for the TMA-fed slab kernels (csrc/slabx.cuh), which serve the (x1, x2) slabs of the
-Si512 (64 x 64) and Si1536 (128 x 48) configs.  A short x0 axis keeps the oracle fast; the cases walk through the
+Si512 (64 x 64), Si1536 (128 x 48), Si216 (48 x 48) and Si64 (32 x 32) configs.  A short x0 axis keeps the oracle fast; the cases walk through the
 paths the full-size runs do not isolate: fewer loop iterations than rotating tiles (1, 2, 3 orbitals per CTA),
 ragged waves, the split i loop of pass A, the conj(W) accumulate of the pair-symmetric schedule, j-blocks.
 
@@ -18,6 +18,8 @@ TOL = 1e-10
 SHAPES = [
     ("s64x64", (11.0, 41.04, 41.04), (16, 64, 64)),        # kind P, bulk stores, three tiles
     ("s128x48", (11.0, 82.08, 30.78), (16, 128, 48)),      # kind Q, 24-point stage, two tiles
+    ("s48x48", (11.0, 30.78, 30.78), (16, 48, 48)),        # kind Q, 9-point stage, 144-task DFT16 stages
+    ("s32x32", (11.0, 20.52, 20.52), (32, 32, 32)),        # kind Q, 4-point stage, 64-task DFT16 stages
 ]
 
 
