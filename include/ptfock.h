@@ -88,7 +88,9 @@ int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const void *psi, 
 
 /* Same as ptfock_apply but phi, psi, out are HOST pointers (pinned memory gives full PCIe speed;
  * pageable works).  The library copies Phi (and Psi) to device buffers it owns, applies, copies the
- * result back, and synchronises `stream`.  n_targets <= max_targets. */
+ * result back, and synchronises `stream`.  The copies run on a stream of the plan's, in chunks of block_i
+ * orbitals, each wave waiting only for the chunks it reads, so most of the transfer overlaps the kernels.
+ * n_targets <= max_targets. */
 int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const void *psi_host, int32_t self_offset,
                       int32_t n_targets, void *out_host, void *stream);
 

@@ -175,6 +175,8 @@ struct ptfock_plan {
     cd *energy_buf;
     // host path staging
     cd *st_phi, *st_psi, *st_out;
+    cudaStream_t copy_stream;           // host path: copies run here, chunk by chunk, overlapped with the waves
+    std::vector<cudaEvent_t> *copy_ev;
     // statistics
     long long last_launches, last_pairs, total_launches;
     int last_symmetric;
@@ -209,6 +211,8 @@ void free_plan(ptfock_plan *p) {
     cudaFree(p->st_psi);
     cudaFree(p->st_out);
     if (p->ev_pool) { for (cudaEvent_t e : *p->ev_pool) cudaEventDestroy(e); delete p->ev_pool; }
+    if (p->copy_ev) { for (cudaEvent_t e : *p->copy_ev) cudaEventDestroy(e); delete p->copy_ev; }
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     delete p->ev_tags;
     delete p;
 }
@@ -484,8 +488,21 @@ int check_apply_args(const ptfock_plan *p, const void *phi, const void *psi, int
     return PTFOCK_OK;
 }
 
+// Host path (ptfock_apply_host): Phi is copied in chunks of `chunk` orbitals on the plan's copy stream, one event per
+// chunk; a wave waits only for the chunks it reads, so the copy of the rest overlaps the first waves.
+struct HostPipe {
+    cudaStream_t cs;
+    std::vector<cudaEvent_t> *ev;       // [0, n_chunks): Phi chunk landed; [n_chunks]: Psi landed; [n_chunks + 1]: scratch event
+    int chunk, n_chunks;
+    std::vector<char> waited;
+    void need(cudaStream_t st, int lo, int hi) {                  // orbitals [lo, hi) of Phi
+        for (int c = lo / chunk; c <= (hi - 1) / chunk && c < n_chunks; ++c)
+            if (!waited[c]) { cudaStreamWaitEvent(st, (*ev)[c], 0); waited[c] = 1; }
+    }
+};
+
 int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, int n_targets, cd *out,
-                 cudaStream_t st) {
+                 cudaStream_t st, HostPipe *hp = nullptr) {
     const size_t gbytes = sizeof(cd) * (size_t)p->N;
     if (n_targets == 0) { p->last_launches = 0; p->last_pairs = 0; p->last_symmetric = 0; return PTFOCK_OK; }
     if (overlaps(out, gbytes * n_targets, phi, gbytes * p->d.n_occ)) return PTFOCK_ERR_ALIAS;
@@ -504,6 +521,7 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
             const int nj = (n_occ - j0 < bs) ? n_occ - j0 : bs;
             for (int i0 = 0; i0 <= j0; i0 += bs) {
                 const int ni = (n_occ - i0 < bs) ? n_occ - i0 : bs;
+                if (hp) { hp->need(st, i0, i0 + ni); hp->need(st, j0, j0 + nj); }
                 wave_forward_mid(w, phi, phi, i0, ni, j0, nj);
                 wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
                 if (i0 != j0) wave_accumulate(w, phi, j0, nj, out, i0, ni, 1, nj, 1);
@@ -511,12 +529,28 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
         }
     } else {
         const cd *tgt = psi ? psi : phi + (size_t)self_offset * p->N;
-        for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
-            const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
+        if (hp) {
+            // host path: i blocks outermost, so every chunk of Phi is used by all j-blocks as soon as it has landed
+            // and the rest of the copy hides behind those waves (out_j accumulates over the waves in any order)
+            if (psi) cudaStreamWaitEvent(st, (*hp->ev)[hp->n_chunks], 0);
+            else hp->need(st, self_offset, self_offset + n_targets);
             for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
                 const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
-                wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
-                wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
+                hp->need(st, i0, i0 + ni);
+                for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
+                    const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
+                    wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
+                    wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
+                }
+            }
+        } else {
+            for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
+                const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
+                for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
+                    const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
+                    wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
+                    wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
+                }
             }
         }
     }
@@ -587,12 +621,43 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     if (rc == PTFOCK_OK) rc = ensure(&plan->st_out, gbytes * plan->d.max_targets);
     if (rc == PTFOCK_OK && psi_host) rc = ensure(&plan->st_psi, gbytes * plan->d.max_targets);
     if (rc != PTFOCK_OK) return rc;
-    CU(cudaMemcpyAsync(plan->st_phi, phi_host, gbytes * plan->d.n_occ, cudaMemcpyHostToDevice, st));
-    if (psi_host) CU(cudaMemcpyAsync(plan->st_psi, psi_host, gbytes * n_targets, cudaMemcpyHostToDevice, st));
-    rc = apply_device(plan, plan->st_phi, psi_host ? plan->st_psi : nullptr, self_offset, n_targets, plan->st_out, st);
-    if (rc != PTFOCK_OK) return rc;
+    if (n_targets == 0) return PTFOCK_OK;
+    if (!plan->copy_stream) CU(cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
+    HostPipe hp;
+    hp.cs = plan->copy_stream;
+    hp.chunk = plan->Ib;
+    hp.n_chunks = (plan->d.n_occ + hp.chunk - 1) / hp.chunk;
+    if (!plan->copy_ev) plan->copy_ev = new std::vector<cudaEvent_t>();
+    while ((int)plan->copy_ev->size() < hp.n_chunks + 2) {
+        cudaEvent_t e;
+        CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        plan->copy_ev->push_back(e);
+    }
+    hp.ev = plan->copy_ev;
+    hp.waited.assign(hp.n_chunks, 0);
+    // the copy stream starts after whatever the caller queued on `stream` (the event slot [n_chunks + 1] is free here)
+    CU(cudaEventRecord((*hp.ev)[hp.n_chunks + 1], st));
+    CU(cudaStreamWaitEvent(hp.cs, (*hp.ev)[hp.n_chunks + 1], 0));
+    if (psi_host) {
+        CU(cudaMemcpyAsync(plan->st_psi, psi_host, gbytes * n_targets, cudaMemcpyHostToDevice, hp.cs));
+        CU(cudaEventRecord((*hp.ev)[hp.n_chunks], hp.cs));
+    }
+    // chunks that hold the targets (Psi = Phi[self_offset...]) go first, the rest in the order the i loop reads them
+    std::vector<int> order;
+    const int t_lo = psi_host ? 0 : self_offset / hp.chunk, t_hi = psi_host ? -1 : (self_offset + n_targets - 1) / hp.chunk;
+    for (int c = t_lo; c <= t_hi; ++c) order.push_back(c);
+    for (int c = 0; c < hp.n_chunks; ++c) if (c < t_lo || c > t_hi) order.push_back(c);
+    for (int c : order) {
+        const int lo = c * hp.chunk, cnt = (plan->d.n_occ - lo < hp.chunk) ? plan->d.n_occ - lo : hp.chunk;
+        CU(cudaMemcpyAsync(plan->st_phi + (size_t)lo * plan->N, (const cd *)phi_host + (size_t)lo * plan->N, gbytes * cnt,
+                           cudaMemcpyHostToDevice, hp.cs));
+        CU(cudaEventRecord((*hp.ev)[c], hp.cs));
+    }
+    rc = apply_device(plan, plan->st_phi, psi_host ? plan->st_psi : nullptr, self_offset, n_targets, plan->st_out, st, &hp);
+    if (rc != PTFOCK_OK) { cudaStreamSynchronize(hp.cs); return rc; }
     CU(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    CU(cudaStreamSynchronize(hp.cs));
     return PTFOCK_OK;
 }
 

@@ -112,6 +112,19 @@ def test_host_path_and_stream(cuda_device):
         s.synchronize()
         torch.cuda.synchronize()
     assert torch.equal(host, ref.cpu()) and torch.equal(on_s, ref)
+    # host path, Psi = Phi: the chunked, overlapped copies (chunk = block_i orbitals) must not change a bit --
+    # symmetric schedule (whole set), a streamed j-block whose targets sit in a later chunk, several j-blocks
+    cfg2 = synth.Config("h2", (10.26,) * 3, (16, 16, 16), 7, synth.KERNEL_COULOMB)
+    phi2 = synth.random_orbitals(cfg2, 3, 7, cuda_device)
+    hphi = phi2.cpu().pin_memory()
+    with binding.plan_for(cfg2, block_i=2, block_j=2) as plan:
+        for off, nt in ((0, 7), (5, 2), (1, 5)):
+            dev = plan.apply(phi2, None, self_offset=off, n_targets=nt)
+            sym = plan.info()["last_symmetric"]
+            host = plan.apply_host(hphi, None, self_offset=off, n_targets=nt)
+            torch.cuda.synchronize()
+            assert sym == (1 if nt == 7 else 0)
+            assert torch.equal(host, dev.cpu()), (off, nt)
 
 
 def test_edge_cases_and_errors(cuda_device):
