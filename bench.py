@@ -259,6 +259,19 @@ def main():
                 "path": {"bytes_per_pair_solve": sum(per_pair), "pairs_per_s_at_peak": peak * 1e9 / sum(per_pair),
                          "frac": (pairs_exec / (ms_step * 1e-3)) / (peak * 1e9 / sum(per_pair)),
                          "survey_72N_frac": (pairs_exec / (ms_step * 1e-3)) / (peak * 1e9 / (72.0 * N))}}
+    # second roof: the plain FP64 pipe, measured live with the library's DFMA loop; nominal flops per
+    # pair-solve F = 2 * 5 N log2 N (forward + inverse FFT) + 16 N (product, x v, x phi + sum)
+    try:
+        import math
+        p64 = binding.measure_fp64_peak(local)
+        flops = 10.0 * N * math.log2(N) + 16.0 * N
+        roofline["fp64"] = {"peak_tflops": p64, "peak_source": "measured live (ptfock_measure_dfma_peak, DFMA loop)",
+                            "nominal_flops_per_pair_solve": flops,
+                            "achieved_tflops": pairs_exec / (ms_step * 1e-3) * flops / 1e12,
+                            "frac": pairs_exec / (ms_step * 1e-3) * flops / 1e12 / p64,
+                            "pairs_per_s_at_peak": p64 * 1e12 / flops}
+    except Exception as e:                      # a measurement aid only: never fail the bench on it
+        roofline["fp64"] = {"error": str(e)}
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             roofline["traffic"] = json.load(f).get(cfg.name, {}).get(names[k])

@@ -121,6 +121,11 @@ int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const void *psi_j, v
 int ptfock_set_profiling(ptfock_plan *plan, int32_t on);
 int ptfock_get_profile(ptfock_plan *plan, double ms[3], int64_t launches[3], int32_t reset);
 
+/* Measurement aid (the path sits under two roofs, HBM bandwidth and the plain FP64 pipe, and
+ * MEASURED_PEAKS.json records no FP64 number): runs a register-resident DFMA loop on `device` (legacy default
+ * stream, synchronous, ~50 ms) and writes the best sustained rate in TFLOP/s (2 flops per DFMA) to HOST memory. */
+int ptfock_measure_dfma_peak(int32_t device, double *tflops_host);
+
 #ifdef __cplusplus
 }
 #endif

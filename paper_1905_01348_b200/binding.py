@@ -20,7 +20,7 @@ KERNEL_HSE = 1
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
-           "ptfock_set_profiling", "ptfock_get_profile"]
+           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -76,6 +76,7 @@ def lib() -> ctypes.CDLL:
         L.ptfock_debug_pair.argtypes = [vp, vp, vp, vp, vp]
         L.ptfock_set_profiling.argtypes = [vp, i32]
         L.ptfock_get_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64), i32]
+        L.ptfock_measure_dfma_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double)]
         for name in EXPORTS:
             if name != "ptfock_strerror":
                 getattr(L, name).restype = ctypes.c_int
@@ -229,6 +230,13 @@ class Plan:
 
     def __exit__(self, *a):
         self.destroy()
+
+
+def measure_fp64_peak(device: int = 0) -> float:
+    """Sustained DFMA rate of the device in TFLOP/s (ptfock_measure_dfma_peak)."""
+    v = ctypes.c_double(0.0)
+    _check(lib().ptfock_measure_dfma_peak(int(device), ctypes.byref(v)), "ptfock_measure_dfma_peak")
+    return v.value
 
 
 def plan_for(cfg, device: int = 0, max_targets: int | None = None, **kw) -> Plan:

@@ -310,6 +310,18 @@ __global__ void __launch_bounds__(PencilShape<N0>::NT, PencilShape<N0>::MINB) pe
     }
 }
 
+// ---- FP64 pipe peak (measurement aid for bench.py: the second roof of SURVEY.md 8(d)) ---------------------------
+// 8 independent register-resident DFMA chains per thread; 2 * 8 * iters flops per thread.
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int k = 0; k < iters; ++k) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    const double r = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (r == 123.456) sink[0] = r;          // never true: keeps the loop alive
+}
+
 // ---- helpers --------------------------------------------------------------------------------------
 // partial[b] = sum over the block's share of conj(psi) * vx
 __global__ void __launch_bounds__(256) dot_partial(const cd *psi, const cd *vx, long long n, double2 *partial) {

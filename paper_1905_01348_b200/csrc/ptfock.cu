@@ -682,6 +682,37 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
     return PTFOCK_OK;
 }
 
+extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
+    if (!tflops_host) return PTFOCK_ERR_INVALID_ARG;
+    CU(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
+    double *sink = nullptr;
+    CU(cudaMalloc(&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 8, iters = 1 << 16;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {             // first repetitions warm the clocks up
+        cudaEventRecord(e0, 0);
+        fp64_peak_kernel<<<blocks, 256>>>(sink, iters, 1.0000001, 1e-9);
+        cudaEventRecord(e1, 0);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; cudaFree(sink); return PTFOCK_ERR_CUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+        if (rep >= 2 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    *tflops_host = best;
+    return PTFOCK_OK;
+}
+
 extern "C" int ptfock_set_profiling(ptfock_plan *plan, int32_t on) {
     if (!plan) return PTFOCK_ERR_INVALID_ARG;
     plan->profiling = on ? 1 : 0;
