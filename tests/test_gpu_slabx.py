@@ -93,3 +93,22 @@ def test_single_pair_W(cuda_device, shape):
         w = plan.debug_pair(ab[0], ab[1]).cpu().numpy()
     ref = -cfg.alpha * oracle.pair_w(cfg.cell, cfg.n, cfg.kernel, cfg.omega, ab[0].cpu().numpy(), ab[1].cpu().numpy())
     assert _rel(w, ref) <= TOL
+
+
+@pytest.mark.parametrize("shape", SHAPES[:2], ids=[s[0] for s in SHAPES[:2]])
+def test_repeated_applies_are_bit_identical(cuda_device, shape):
+    """No atomics anywhere on the path, so every apply must reproduce the same bits; a shared-memory / bulk-copy
+    hazard in the rotating tiles (compute-sanitizer is closed on this pool) would show up as run-to-run noise.
+    40 orbitals per CTA loop = many trips around the tile ring; sampled columns also checked against the oracle."""
+    name, edges, n = shape
+    cfg = synth.Config(name, edges, n, 40, synth.KERNEL_HSE, separate_psi=True)
+    phi = synth.random_orbitals(cfg, 31, 40, cuda_device)
+    psi = synth.random_orbitals(cfg, 32, 9, cuda_device)
+    with binding.plan_for(cfg, max_targets=9) as plan:
+        first = plan.apply(phi, psi).clone()
+        for _ in range(4):
+            again = plan.apply(phi, psi)
+            torch.cuda.synchronize()
+            assert torch.equal(first, again)
+    ref = _oracle(cfg, phi, psi[[0, 8]].contiguous())
+    assert _rel(first[[0, 8]].cpu().numpy(), ref) <= TOL
