@@ -31,6 +31,9 @@ if ROOT not in sys.path:
 METRIC = "Fock exchange pair-FFTs/s (fp64, 1 B200) and % of HBM roofline"
 UNIT = "pair-FFTs/s"
 HBM_FALLBACK_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# BASELINE.md holds a paper number only for the paper's own workload (3072 orbitals on the 60 x 90 x 120 grid):
+# 2881 pair-solves/s per V100, computation only (derived from PAPER.md:299, Table 1, 36 GPUs).  Another machine's: context.
+PAPER_PAIRS_PER_S = {"Si1536p": 2881.0}
 
 
 def load_peak():
@@ -323,7 +326,8 @@ def main():
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "vs_baseline": (value / world / PAPER_PAIRS_PER_S[cfg.name]) if cfg.name in PAPER_PAIRS_PER_S else None,
+                "dtype": "f64", "data": "synthetic",
                 "config": {"workload": wl, "grid": list(cfg.n), "n_i": n_i, "n_j": n_j,
                            "kernel": "HSE" if cfg.kernel == 1 else "Coulomb",
                            "pair_solves_executed_per_step": pairs_exec, "symmetric_schedule": bool(info1["last_symmetric"]),

@@ -1,4 +1,4 @@
-// codelets.cuh -- register-resident radix-R complex fp64 DFT butterflies (R = 2, 3, 4, 8, 16).
+// codelets.cuh -- register-resident radix-R complex fp64 DFT butterflies (R = 2, 3, 4, 5, 6, 8, 15, 16).
 //
 // Building blocks of the hand-written FFT passes (BASELINE.json north_star (1): "radix-2/3/4/8/16
 // stages").  Each codelet transforms R values held in registers IN PLACE and leaves them in NATURAL
@@ -56,6 +56,70 @@ template <bool INV> struct DFT<3, INV> {
         v[0] = cadd(v[0], t);
         v[1] = cadd(m, u);
         v[2] = csub(m, u);
+    }
+};
+
+// radix 5 (the paper's own grid 60 x 90 x 120, needs the factor 5)
+constexpr double kCos2Pi5 = 0.30901699437494742410229341718282;
+constexpr double kCos4Pi5 = -0.80901699437494742410229341718282;
+constexpr double kSin2Pi5 = 0.95105651629515357211643933337938;
+constexpr double kSin4Pi5 = 0.58778525229247312916870595463907;
+
+template <bool INV> struct DFT<5, INV> {
+    static PTF_DEV void run(cd &x0, cd &x1, cd &x2, cd &x3, cd &x4) {
+        const cd t1 = cadd(x1, x4), t2 = cadd(x2, x3), t3 = csub(x1, x4), t4 = csub(x2, x3);
+        const cd m1 = make_double2(x0.x + kCos2Pi5 * t1.x + kCos4Pi5 * t2.x, x0.y + kCos2Pi5 * t1.y + kCos4Pi5 * t2.y);
+        const cd m2 = make_double2(x0.x + kCos4Pi5 * t1.x + kCos2Pi5 * t2.x, x0.y + kCos4Pi5 * t1.y + kCos2Pi5 * t2.y);
+        // s1 = sin(2pi/5) t3 + sin(4pi/5) t4,  s2 = sin(4pi/5) t3 - sin(2pi/5) t4;  X1,4 = m1 -/+ i s1,  X2,3 = m2 -/+ i s2
+        const cd s1 = mul_mi<INV>(make_double2(kSin2Pi5 * t3.x + kSin4Pi5 * t4.x, kSin2Pi5 * t3.y + kSin4Pi5 * t4.y));
+        const cd s2 = mul_mi<INV>(make_double2(kSin4Pi5 * t3.x - kSin2Pi5 * t4.x, kSin4Pi5 * t3.y - kSin2Pi5 * t4.y));
+        x0 = make_double2(x0.x + t1.x + t2.x, x0.y + t1.y + t2.y);
+        x1 = cadd(m1, s1);
+        x4 = csub(m1, s1);
+        x2 = cadd(m2, s2);
+        x3 = csub(m2, s2);
+    }
+    static PTF_DEV void run(cd (&v)[5]) { run(v[0], v[1], v[2], v[3], v[4]); }
+};
+
+// radix 6 = 2 x 3 and radix 15 = 3 x 5 by the prime-factor (Good-Thomas) map: coprime factors need no twiddles.
+//   n = (N2 n1 + N1 n2) mod N,  k = (c1 k1 + c2 k2) mod N  with c1 = 1 mod N1, 0 mod N2 and c2 = 0 mod N1, 1 mod N2.
+template <bool INV> struct DFT<6, INV> {
+    static PTF_DEV void run(cd (&v)[6]) {
+        // n = 3 n1 + 2 n2 (n1 < 2, n2 < 3); k = 3 k1 + 4 k2 mod 6
+        cd a[2][3];
+#pragma unroll
+        for (int n1 = 0; n1 < 2; ++n1)
+#pragma unroll
+            for (int n2 = 0; n2 < 3; ++n2) a[n1][n2] = v[(3 * n1 + 2 * n2) % 6];
+#pragma unroll
+        for (int n1 = 0; n1 < 2; ++n1) DFT<3, INV>::run(a[n1]);
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) {
+            const cd e = a[0][k2], o = a[1][k2];
+            v[(4 * k2) % 6] = cadd(e, o);
+            v[(3 + 4 * k2) % 6] = csub(e, o);
+        }
+    }
+};
+
+template <bool INV> struct DFT<15, INV> {
+    static PTF_DEV void run(cd (&v)[15]) {
+        // n = 5 n1 + 3 n2 (n1 < 3, n2 < 5); k = 10 k1 + 6 k2 mod 15
+        cd a[3][5];
+#pragma unroll
+        for (int n1 = 0; n1 < 3; ++n1)
+#pragma unroll
+            for (int n2 = 0; n2 < 5; ++n2) a[n1][n2] = v[(5 * n1 + 3 * n2) % 15];
+#pragma unroll
+        for (int n1 = 0; n1 < 3; ++n1) DFT<5, INV>::run(a[n1]);
+#pragma unroll
+        for (int k2 = 0; k2 < 5; ++k2) {
+            cd c[3] = { a[0][k2], a[1][k2], a[2][k2] };
+            DFT<3, INV>::run(c);
+#pragma unroll
+            for (int k1 = 0; k1 < 3; ++k1) v[(10 * k1 + 6 * k2) % 15] = c[k1];
+        }
     }
 };
 

@@ -23,6 +23,7 @@ template <> struct Split<32> { static constexpr int R1 = 8, R2 = 4; };
 template <> struct Split<48> { static constexpr int R1 = 16, R2 = 3; };
 template <> struct Split<64> { static constexpr int R1 = 8, R2 = 8; };
 template <> struct Split<128> { static constexpr int R1 = 16, R2 = 8; };
+template <> struct Split<120> { static constexpr int R1 = 15, R2 = 8; };   // paper grid (NEXT-2): pencil axis only
 
 constexpr int kSlabThreads = 256;
 
@@ -230,7 +231,7 @@ template <int N0> struct PencilShape {
     static constexpr int R1 = Split<N0>::R1, R2 = Split<N0>::R2;
     static constexpr int NT = (R2 == 1) ? 128 : (N0 == 128 ? PTF_PENCIL128_NT : 256);
     static constexpr int SMEM_BYTES = (R2 == 1) ? 0 : (N0 * CW + N0) * (int)sizeof(cd);
-    static constexpr int MINB = (N0 == 128) ? 512 / NT : (R2 == 1 ? 1 : PTF_PENCIL_MINB);   // 128: two CTAs (128 regs) share an SM
+    static constexpr int MINB = (N0 == 128) ? 512 / NT : (R2 == 1 ? 1 : (R1 >= 15 ? 2 : PTF_PENCIL_MINB));   // 128: two CTAs (128 regs) share an SM
 };
 
 struct PencilArgs {
@@ -268,12 +269,14 @@ __global__ void __launch_bounds__(PencilShape<N0>::NT, PencilShape<N0>::MINB) pe
         for (int t = tid; t < N0; t += NT) tw[t] = g.tw0[t];
         __syncthreads();
         const long long p0 = (long long)blockIdx.x * CW;
+        const int cvalid = (sp - p0 < CW) ? (int)(sp - p0) : CW;      // ragged last tile (slab_pts % CW != 0)
         // stage 1: global -> registers -> DFT over a -> twiddle -> shared
         for (int t = tid; t < CW * R2; t += NT) {
             const int c = t % CW, b = t / CW;
             cd v[R1];
 #pragma unroll
-            for (int a = 0; a < R1; ++a) v[a] = base[(long long)(a * R2 + b) * sp + p0 + c];
+            for (int a = 0; a < R1; ++a)
+                v[a] = c < cvalid ? base[(long long)(a * R2 + b) * sp + p0 + c] : make_double2(0.0, 0.0);
             DFT<R1, false>::run(v);
 #pragma unroll
             for (int k1 = 1; k1 < R1; ++k1) v[k1] = cmul(v[k1], tw[b * k1]);
@@ -289,7 +292,8 @@ __global__ void __launch_bounds__(PencilShape<N0>::NT, PencilShape<N0>::MINB) pe
             for (int b = 0; b < R2; ++b) v[b] = s[(k1 * R2 + b) * CW + c];
             DFT<R2, false>::run(v);
 #pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) v[k2] = cscale(v[k2], __ldg(g.v + (long long)(k1 * R2 + k2) * sp + p0 + c));
+            for (int k2 = 0; k2 < R2; ++k2)
+                v[k2] = cscale(v[k2], c < cvalid ? __ldg(g.v + (long long)(k1 * R2 + k2) * sp + p0 + c) : 0.0);
             DFT<R2, true>::run(v);
 #pragma unroll
             for (int b = 0; b < R2; ++b) s[(k1 * R2 + b) * CW + c] = v[b];
@@ -304,8 +308,10 @@ __global__ void __launch_bounds__(PencilShape<N0>::NT, PencilShape<N0>::MINB) pe
 #pragma unroll
             for (int k1 = 1; k1 < R1; ++k1) v[k1] = cmulc(v[k1], tw[b * k1]);
             DFT<R1, true>::run(v);
+            if (c < cvalid) {
 #pragma unroll
-            for (int a = 0; a < R1; ++a) base[(long long)(a * R2 + b) * sp + p0 + c] = v[a];
+                for (int a = 0; a < R1; ++a) base[(long long)(a * R2 + b) * sp + p0 + c] = v[a];
+            }
         }
     }
 }

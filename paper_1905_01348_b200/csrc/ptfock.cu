@@ -39,7 +39,7 @@ template <int N1, int N2> void launch_slab_inv(const SlabArgs &a, dim3 grid, cud
 }
 template <int N0> void launch_pencil(const PencilArgs &a, int pairs, cudaStream_t st) {
     using S = PencilShape<N0>;
-    const int gx = (S::R2 == 1) ? (a.slab_pts + S::NT - 1) / S::NT : a.slab_pts / S::CW;
+    const int gx = (S::R2 == 1) ? (a.slab_pts + S::NT - 1) / S::NT : (a.slab_pts + S::CW - 1) / S::CW;
     pencil_mid<N0><<<dim3(gx, pairs), S::NT, S::SMEM_BYTES, st>>>(a);
 }
 
@@ -97,6 +97,7 @@ typedef SX<128, 48, 16, 8, 3, 16, false, false> SX_128x48;    // kind P: 384 thr
 #endif
 typedef SX<48, 48, 3, 16, 3, 16, true, false> SX_48x48;        // kind Q: 9-point first stage, 144-task DFT16 stages
 typedef SX<32, 32, 2, 16, 2, 16, true, false> SX_32x32;
+typedef SX<90, 60, 6, 15, 4, 15, true, false> SX_90x60;        // paper grid 120 x 90 x 60: 24-point first stage, DFT15 stages
 #define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3, 0 }
 //            N1   N2  A1  B1  A2  B2  min CTAs/SM
 typedef Slab2<64, 64, 4, 16, 16, 4, 1> S2_64x64;
@@ -109,7 +110,7 @@ typedef Slab2<32, 32, 2, 16, 16, 2, 8> S2_32x32;
                        Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2, 0, 1 }
 // first match wins: the 3-stage kernels serve the BASELINE shapes, the generic 4-stage ones the rest
 const SlabEntry kSlabs[] = {
-    SLABX(SX_64x64), SLABX(SX_128x48), SLABX(SX_48x48), SLABX(SX_32x32),
+    SLABX(SX_64x64), SLABX(SX_128x48), SLABX(SX_48x48), SLABX(SX_32x32), SLABX(SX_90x60),
     SLAB2(S2_64x64), SLAB2(S2_128x48), SLAB2(S2_48x48), SLAB2(S2_32x32),
     SLAB(16, 16), SLAB(32, 32), SLAB(48, 48), SLAB(64, 64), SLAB(128, 48),
     SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),
@@ -128,7 +129,7 @@ template <int N0> cudaError_t prepare_pencil() {
                                 PencilShape<N0>::SMEM_BYTES);
 }
 #define PENCIL(N0) { N0, launch_pencil<N0>, prepare_pencil<N0> }
-const PencilEntry kPencils[] = { PENCIL(16), PENCIL(32), PENCIL(48), PENCIL(64), PENCIL(128) };
+const PencilEntry kPencils[] = { PENCIL(16), PENCIL(32), PENCIL(48), PENCIL(64), PENCIL(128), PENCIL(120) };
 #undef PENCIL
 
 // position -> frequency index of the digit-permuted order the forward passes leave an axis in
@@ -142,6 +143,7 @@ void pencil_split(int n, int &r1, int &r2) {
         case 32: r1 = Split<32>::R1; r2 = Split<32>::R2; break;
         case 48: r1 = Split<48>::R1; r2 = Split<48>::R2; break;
         case 64: r1 = Split<64>::R1; r2 = Split<64>::R2; break;
+        case 120: r1 = Split<120>::R1; r2 = Split<120>::R2; break;
         default: r1 = Split<128>::R1; r2 = Split<128>::R2; break;
     }
 }
@@ -192,7 +194,7 @@ struct ptfock_plan {
 // ================================================================================================
 namespace {
 
-const int kEdges[] = { 16, 32, 48, 64, 128 };
+const int kEdges[] = { 16, 32, 48, 64, 128, 60, 90, 120 };     // 60/90/120: only as the paper grid's roles (slab 90x60, pencil 120)
 bool edge_ok(int n) {
     for (int e : kEdges) if (e == n) return true;
     return false;

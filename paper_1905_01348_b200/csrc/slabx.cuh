@@ -40,8 +40,8 @@ struct SX {
     static constexpr int CB1 = Q ? B2 : N2;                 // stage-1 tasks: (b1, cb)
     static constexpr int CB2 = Q ? N2 : B2;                 // stage-2 tasks: (k1a, cb)
     static constexpr int NT1 = B1 * CB1, NT2 = A1 * CB2, NT3 = N1 * A2;
-    static constexpr int NT = NT1;                          // stage 1 has one task per thread
-    static_assert(NT % 32 == 0 && NT <= 512 && (Q || NT2 <= NT), "bad thread count");
+    static constexpr int NT = (NT1 + 31) / 32 * 32;         // stage 1: one task per thread (threads >= NT1 sit it out)
+    static_assert(NT <= 512 && (Q || NT2 <= NT), "bad thread count");
     static constexpr int PM = NT3 + 1;                      // pass C tile (free layout): [m][k2a][k1], odd pitch
     static constexpr int TILE_A = A1 * (B1 * N2 + 1), TILE_C = TS ? TILE_A : B2 * PM;   // elements (Addr below)
     static constexpr int MAXSM = 232448 - 64;
@@ -221,17 +221,19 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
     // stage-1 task of this thread: psi_j values in registers for the whole loop
     const int cb = tid % S::CB1, b1 = tid / S::CB1;
     const int base1 = s1_base<S, false>(tid);
+    const bool act1 = S::NT1 == NT || tid < S::NT1;      // this thread owns a stage-1 task
     cd pj[R1 * C1];
-    {
+    if (act1) {
         const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + slab_off + b1 * N2 + cb;
         tile_load<R1, C1, B1 * N2, B2>(pj, psi);
     }
     cd twr[S::NTWR], twc[S::NTWC];
-    load_twiddles<S>(g.tw1, g.tw2, (S::Q || tid < S::NT2) ? tid : 0, twr, twc);
+    load_twiddles<S>(g.tw1, g.tw2, (S::Q ? act1 : tid < S::NT2) ? tid : 0, twr, twc);
     const int base2 = s2_base<S, false>(tid);            // P: the twiddled stage-2 task of this thread
 
     // ---- stage 1: rho = psi_j conj(phi_i), DFT over a1 (Q: and a2, with both twiddles), in place
     auto stage1 = [&](cd *T) {
+        if (!act1) return;
         cd u[R1 * C1];
         tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
 #pragma unroll
@@ -387,6 +389,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
     const int cb = tid % S::CB1, b1 = tid / S::CB1;
     const int base1 = s1_base<S, CL>(tid);
     const cd *phi0 = g.a + (long long)g.a0 * g.grid_pts + slab_off + b1 * N2 + cb;
+    const bool act1 = S::NT1 == NT || tid < S::NT1;      // this thread owns a last-stage task (and its accumulators)
     cd acc[R1 * C1];
 #pragma unroll
     for (int k = 0; k < R1 * C1; ++k) acc[k] = make_double2(0.0, 0.0);
@@ -456,6 +459,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
     };
     // ---- stage 3' (Q): 2-D inverse over (k1a, k2a); phi_i is fetched column block by column block
     auto stage3i_q = [&](cd *T, const cd *phi, cd (&f)[R1]) {
+        if (!act1) return;
         cd u[R1 * C1];
         tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
 #pragma unroll
@@ -506,7 +510,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
         __syncthreads();
         if (tid < 32 && it + NBUF - 1 < n_it) refill(it + NBUF - 1);
         cd fq[S::Q ? R1 : 1];
-        if (S::Q) {     // first column block of phi_i: in flight during stage 2'
+        if (S::Q && act1) {     // first column block of phi_i: in flight during stage 2'
 #pragma unroll
             for (int r = 0; r < R1; ++r) fq[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2));
         }
@@ -556,6 +560,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
             }
         }
     }
+    if (!act1) return;
     cd *o = g.out + (long long)(g.b0 + tt) * g.grid_pts + slab_off + b1 * N2 + cb;
 #pragma unroll
     for (int r = 0; r < R1; ++r)

@@ -68,6 +68,9 @@ CONFIGS = {
     "Si216": Config("Si216", (3 * A_SI,) * 3, (48, 48, 48), 432, KERNEL_HSE),
     "Si512": Config("Si512", (4 * A_SI,) * 3, (64, 64, 64), 1024, KERNEL_HSE, separate_psi=True),
     "Si1536": Config("Si1536", (8 * A_SI, 8 * A_SI, 3 * A_SI), (128, 128, 48), 3072, KERNEL_HSE, j_block=96),
+    # the paper's own 1536-atom workload (4 x 6 x 8 cell, wavefunction grid
+    # 60 x 90 x 120 = 648 000 points, 3072 orbitals), axes ordered so that the 120-point edge is x0 (the pencil axis)
+    "Si1536p": Config("Si1536p", (8 * A_SI, 6 * A_SI, 4 * A_SI), (120, 90, 60), 3072, KERNEL_HSE, j_block=96),
 }
 
 _M64 = (1 << 64) - 1

@@ -33,6 +33,8 @@ SMALL = [
     ("g64x48x32", (30.0, 22.0, 16.0), (64, 48, 32), 2, synth.KERNEL_HSE, True),
     ("g128x32x64", (50.0, 16.0, 30.0), (128, 32, 64), 2, synth.KERNEL_HSE, True),
     ("g32x128x48", (16.0, 50.0, 22.0), (32, 128, 48), 2, synth.KERNEL_COULOMB, False),
+    ("g120x16x16", (82.08, 10.26, 10.26), (120, 16, 16), 3, synth.KERNEL_HSE, True),     # radix-15 pencil (paper grid)
+    ("g120x90x60", (82.08, 61.56, 41.04), (120, 90, 60), 2, synth.KERNEL_HSE, False),    # the paper's 60x90x120 grid
 ]
 
 

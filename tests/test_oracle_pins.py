@@ -210,7 +210,7 @@ def test_T5_energy_real_and_nonpositive(kernel):
 
 
 # --------------------------------------------------------------------------------------- T6
-@pytest.mark.parametrize("nlen", [1, 2, 3, 4, 6, 8, 9, 12, 16, 32, 48, 64, 128, 5, 10])
+@pytest.mark.parametrize("nlen", [1, 2, 3, 4, 6, 8, 9, 12, 16, 32, 48, 64, 128, 5, 10, 15, 60, 90, 120])
 def test_T6_fft1d_matches_definition(nlen):
     rng = _rng(nlen)
     x = _randc(rng, (nlen,))
@@ -232,7 +232,7 @@ def test_T6_fft1d_matches_definition(nlen):
     assert np.abs(spec - e).max() <= 1e-13 * nlen
 
 
-@pytest.mark.parametrize("n", [(4, 6, 8), (16, 16, 16), (12, 8, 3)])
+@pytest.mark.parametrize("n", [(4, 6, 8), (16, 16, 16), (12, 8, 3), (10, 15, 6)])
 def test_T6_fft3d_roundtrip_parseval_and_definition(n):
     rng = _rng(sum(n))
     x = _randc(rng, n)
