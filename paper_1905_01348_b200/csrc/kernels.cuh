@@ -227,11 +227,11 @@ template <int N0> struct PencilShape {
 #ifndef PTF_PENCIL128_NT
 #define PTF_PENCIL128_NT (PTF_PENCIL128_CW * 8)
 #endif
-    static constexpr int CW = (N0 == 128) ? PTF_PENCIL128_CW : PTF_PENCIL_CW;      // contiguous slab positions per CTA
+    static constexpr int CW = (N0 >= 120) ? PTF_PENCIL128_CW : PTF_PENCIL_CW;      // contiguous slab positions per CTA
     static constexpr int R1 = Split<N0>::R1, R2 = Split<N0>::R2;
-    static constexpr int NT = (R2 == 1) ? 128 : (N0 == 128 ? PTF_PENCIL128_NT : 256);
+    static constexpr int NT = (R2 == 1) ? 128 : (N0 >= 120 ? PTF_PENCIL128_NT : 256);
     static constexpr int SMEM_BYTES = (R2 == 1) ? 0 : (N0 * CW + N0) * (int)sizeof(cd);
-    static constexpr int MINB = (N0 == 128) ? 512 / NT : (R2 == 1 ? 1 : (R1 >= 15 ? 2 : PTF_PENCIL_MINB));   // 128: two CTAs (128 regs) share an SM
+    static constexpr int MINB = (N0 >= 120) ? 512 / NT : (R2 == 1 ? 1 : PTF_PENCIL_MINB);   // 128: two CTAs (128 regs) share an SM
 };
 
 struct PencilArgs {
