@@ -95,8 +95,11 @@ typedef SX<128, 48, 8, 16, 3, 16, true, false> SX_128x48;     // kind Q: 256 thr
 #else
 typedef SX<128, 48, 16, 8, 3, 16, false, false> SX_128x48;    // kind P: 384 threads, 24-point middle stage (spills: slower)
 #endif
-typedef SX<48, 48, 3, 16, 3, 16, true, false> SX_48x48;        // kind Q: 9-point first stage, 144-task DFT16 stages
-typedef SX<32, 32, 2, 16, 2, 16, true, false> SX_32x32;
+#ifndef PTF_SMALL_MINB
+#define PTF_SMALL_MINB 2      // 36 KB / 16 KB tiles: two CTAs per SM (128 registers) run out of phase
+#endif
+typedef SX<48, 48, 3, 16, 3, 16, true, false, PTF_SMALL_MINB> SX_48x48;        // kind Q: 9-point first stage, 144-task DFT16 stages
+typedef SX<32, 32, 2, 16, 2, 16, true, false, PTF_SMALL_MINB> SX_32x32;
 typedef SX<90, 60, 6, 15, 4, 15, true, false> SX_90x60;        // paper grid 120 x 90 x 60: 24-point first stage, DFT15 stages
 #define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3, 0 }
 //            N1   N2  A1  B1  A2  B2  min CTAs/SM

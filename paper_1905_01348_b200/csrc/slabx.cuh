@@ -29,8 +29,9 @@ namespace ptfock {
 // TS_: pass A hands its finished tile to bulk async STORES (the scratch slab is then the tile's own order,
 // [pos1][pos2], and pass C works in the pass A layout); otherwise stage 3 stores from registers in the free
 // layout above.  Needs three rotating tiles (the store has to drain before the tile is refilled).
-template <int N1_, int N2_, int A1_, int B1_, int A2_, int B2_, bool Q_, bool TS_>
+template <int N1_, int N2_, int A1_, int B1_, int A2_, int B2_, bool Q_, bool TS_, int MINB_ = 1>
 struct SX {
+    static constexpr int MINB = MINB_;                      // CTAs per SM the register budget is capped for
     static constexpr int N1 = N1_, N2 = N2_, A1 = A1_, B1 = B1_, A2 = A2_, B2 = B2_;
     static constexpr bool Q = Q_, TS = TS_, CLAYOUT = !TS_;
     static_assert(A1 * B1 == N1 && A2 * B2 == N2, "bad split");
@@ -192,7 +193,7 @@ PTF_DEV void issue_blocks(cd *tile, const cd *src, unsigned long long *bar, int 
 // ---- pass A ---------------------------------------------------------------------------------------
 // grid = (targets in the wave, n0, chunks of the i loop)
 template <class S>
-__global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
+__global__ void __launch_bounds__(S::NT, S::MINB) slabx_fwd(const SlabArgs g) {
     constexpr int N2 = S::N2, B1 = S::B1, B2 = S::B2, R1 = S::R1, C1 = S::C1, R2 = S::R2, C2 = S::C2;
     constexpr int NT = S::NT, NBUF = S::NBUF_A, TILE = S::TILE_A;
     using A = Addr<S, false>;
@@ -357,7 +358,7 @@ __global__ void __launch_bounds__(S::NT, 1) slabx_fwd(const SlabArgs g) {
 // ---- pass C ---------------------------------------------------------------------------------------
 // grid = (targets, n0): out[b0+tt] += sum_ss a[a0+ss] * W[ss*stride_loop + tt*stride_cta]   (W or conj(W))
 template <class S>
-__global__ void __launch_bounds__(S::NT, 1) slabx_inv_acc(const SlabArgs g) {
+__global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g) {
     constexpr int N2 = S::N2, B1 = S::B1, B2 = S::B2, R1 = S::R1, C1 = S::C1, R2 = S::R2, C2 = S::C2;
     constexpr int NT = S::NT, NBUF = S::NBUF_C, TILE = S::TILE_C;
     constexpr bool CL = S::CLAYOUT;
