@@ -5,6 +5,7 @@
 #include "kernels.cuh"
 #include "slab2.cuh"
 #include "slabx.cuh"
+#include "pencil_tma.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -121,18 +122,32 @@ const SlabEntry kSlabs[] = {
 #undef SLAB
 #undef SLAB2
 
+typedef void (*pencil_tma_launch_fn)(const CUtensorMap &, const PencilTmaArgs &, int pairs, cudaStream_t);
 struct PencilEntry {
     int n0;
     pencil_launch_fn run;
     cudaError_t (*prepare)();
+    pencil_tma_launch_fn run_tma;       // tensor-map TMA variant (pencil_tma.cuh); null for single-stage pencils
+    cudaError_t (*prepare_tma)();
+    int tma_cw;
 };
+template <int N0> void launch_pencil_tma(const CUtensorMap &m, const PencilTmaArgs &a, int pairs, cudaStream_t st) {
+    using S = PencilTma<N0>;
+    pencil_tma<N0><<<dim3((a.slab_pts + S::CW - 1) / S::CW, pairs), S::NT, S::SMEM_BYTES, st>>>(m, a);
+}
+template <int N0> cudaError_t prepare_pencil_tma() {
+    return cudaFuncSetAttribute(pencil_tma<N0>, cudaFuncAttributeMaxDynamicSharedMemorySize, PencilTma<N0>::SMEM_BYTES);
+}
 template <int N0> cudaError_t prepare_pencil() {
     if (PencilShape<N0>::SMEM_BYTES <= 48 * 1024) return cudaSuccess;
     return cudaFuncSetAttribute(pencil_mid<N0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 PencilShape<N0>::SMEM_BYTES);
 }
-#define PENCIL(N0) { N0, launch_pencil<N0>, prepare_pencil<N0> }
-const PencilEntry kPencils[] = { PENCIL(16), PENCIL(32), PENCIL(48), PENCIL(64), PENCIL(128), PENCIL(120) };
+#define PENCIL(N0) { N0, launch_pencil<N0>, prepare_pencil<N0>, launch_pencil_tma<N0>, prepare_pencil_tma<N0>, PencilTma<N0>::CW }
+#define PENCIL_REG(N0) { N0, launch_pencil<N0>, prepare_pencil<N0>, nullptr, nullptr, 0 }
+// the tensor-map variant serves the long pencils; at n0 <= 48 its 16-wide tiles leave most threads idle (measured slower)
+const PencilEntry kPencils[] = { PENCIL_REG(16), PENCIL_REG(32), PENCIL_REG(48), PENCIL(64), PENCIL(128), PENCIL(120) };
+#undef PENCIL_REG
 #undef PENCIL
 
 // position -> frequency index of the digit-permuted order the forward passes leave an axis in
@@ -185,6 +200,8 @@ struct ptfock_plan {
     // statistics
     long long last_launches, last_pairs, total_launches;
     int last_symmetric;
+    CUtensorMap tmap;                   // pair scratch as [pairs*n0 rows][2*slab_pts doubles] (pass B, TMA variant)
+    int use_tma;
     // optional per-pass device timing (ptfock_set_profiling): events bracket every launch
     int profiling;
     std::vector<cudaEvent_t> *ev_pool;
@@ -367,6 +384,31 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     p->Jb = Jb;
     p->scratch_bytes = (size_t)Ib * Jb * pair_bytes;
     CUP(cudaMalloc(&p->scratch, p->scratch_bytes));
+    p->use_tma = 0;
+    {
+        const char *pk = std::getenv("PTFOCK_PENCIL");          // "legacy": the register-path pencil kernel (comparison runs)
+        if (pencil->run_tma && !(pk && std::strcmp(pk, "legacy") == 0)) {
+            typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                          const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                          CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+            void *fn = nullptr;
+            cudaDriverEntryPointQueryResult qres;
+            CUP(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+            if (fn && qres == cudaDriverEntryPointSuccess) {
+                const cuuint64_t dims[2] = { (cuuint64_t)2 * p->slab_pts, (cuuint64_t)Ib * Jb * d.n[0] };
+                const cuuint64_t strides[1] = { (cuuint64_t)p->slab_pts * sizeof(cd) };
+                const cuuint32_t box[2] = { (cuuint32_t)(2 * pencil->tma_cw), (cuuint32_t)d.n[0] };
+                const cuuint32_t estr[2] = { 1, 1 };
+                CUresult r = ((encode_fn)fn)(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
+                                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                if (r == CUDA_SUCCESS) {
+                    CUP(pencil->prepare_tma());
+                    p->use_tma = 1;
+                }
+            }
+        }
+    }
     CUP(cudaMalloc(&p->partials, sizeof(double2) * 1024));
     CUP(cudaMalloc(&p->result_dev, sizeof(double2)));
     CUP(cudaMallocHost(&p->result_host, sizeof(double2)));
@@ -456,9 +498,15 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
     mark(w, -1);
     p->slab->fwd(a, dim3(nj, p->d.n[0], z), w.st);
     mark(w, 0);
-    PencilArgs b;
-    b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
-    p->pencil->run(b, ni * nj, w.st);
+    if (p->use_tma) {
+        PencilTmaArgs b;
+        b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
+        p->pencil->run_tma(p->tmap, b, ni * nj, w.st);
+    } else {
+        PencilArgs b;
+        b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
+        p->pencil->run(b, ni * nj, w.st);
+    }
     mark(w, 1);
     w.launches += 2;
     w.pairs += (long long)ni * nj;
