@@ -15,6 +15,7 @@ T8 structure: W_ji = conj(W_ij), column subsets, linearity, real orbitals, grid 
 All CPU, all small: the whole file runs in well under a minute.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -324,3 +325,23 @@ def test_oracle_rejects_bad_arguments():
         oracle.apply(CELLS["ortho"], n, HSE, OMEGA, 1.0, phi, cols=[1])
     with pytest.raises(TypeError):
         oracle.apply(CELLS["ortho"], n, HSE, OMEGA, 1.0, phi.astype(np.complex64))
+
+
+# --------------------------------------------------------------------------------------- golden table
+def test_golden_vg_table_pins_the_oracle_kernel():
+    """tests/golden/vg_table.txt: v(G) in 40-digit decimal arithmetic (written by tests/golden/make_vg_table.py from the
+    BASELINE.json north_star formulas), including both G = 0 conventions (readings Q2, Q3).  The
+    oracle's table must agree to a few ulp at every listed (cell, m), for both kernels."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "vg_table.txt")
+    rows = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 2 * 3 * 10
+    n = (32, 32, 32)
+    cache = {}
+    for kernel, _cell, l0, l1, l2, m0, m1, m2, val in rows:
+        key = (kernel, l0, l1, l2)
+        if key not in cache:
+            cell = [float(l0), 0, 0, 0, float(l1), 0, 0, 0, float(l2)]
+            cache[key] = oracle.vtable(cell, n, COUL if kernel == "coulomb" else HSE, 0.106)
+        got = cache[key][int(m0) % n[0], int(m1) % n[1], int(m2) % n[2]]
+        want = float(val)
+        assert abs(got - want) <= 1e-14 * max(abs(want), 1e-300), (kernel, l0, m0, m1, m2, got, want)
