@@ -377,6 +377,8 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (Jb > d.max_targets) Jb = d.max_targets;
     const size_t pair_bytes = sizeof(cd) * (size_t)p->N;
     const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)6 << 30);
+    while ((long long)Ib * Jb > 65535 && Ib > 1) Ib = (Ib + 1) / 2;     // pass B puts the wave's pairs on gridDim.y
+    while ((long long)Ib * Jb > 65535 && Jb > 1) Jb = (Jb + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Jb > 1) Jb = (Jb + 1) / 2;
     if ((size_t)Ib * Jb * pair_bytes > limit) { free_plan(p); return PTFOCK_ERR_ALLOC; }

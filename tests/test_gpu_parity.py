@@ -159,3 +159,19 @@ def test_edge_cases_and_errors(cuda_device):
     with binding.plan_for(cfg1) as plan:
         o1 = plan.apply(p1)
     assert _rel(o1.cpu().numpy(), _oracle(cfg1, p1)) <= TOL
+
+
+def test_oversized_tile_is_clamped(cuda_device):
+    """block_i x block_j beyond what one launch can index (pass B: pairs on gridDim.y <= 65535) is reduced at plan
+    creation instead of failing at launch."""
+    cfg = synth.Config("big", (10.26,) * 3, (16, 16, 16), 300, synth.KERNEL_HSE, separate_psi=True)
+    phi = synth.random_orbitals(cfg, 7, 300, cuda_device)
+    psi = synth.random_orbitals(cfg, 8, 300, cuda_device)
+    with binding.plan_for(cfg, block_i=300, block_j=300) as plan:
+        info = plan.info()
+        assert info["block_i"] * info["block_j"] <= 65535
+        out = plan.apply(phi, psi)
+        torch.cuda.synchronize()
+    cols = [0, 149, 299]
+    ref = _oracle(cfg, phi, psi[cols].contiguous())
+    assert _rel(out[cols].cpu().numpy(), ref) <= TOL
