@@ -571,7 +571,7 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
         // square blocks; block pair (bi <= bj): W_ij for i in bi, j in bj serves out_j (as is) and, off the
         // diagonal, out_i through W_ji = conj(W_ij) (v real and even).
         int bs = p->Ib < p->Jb ? p->Ib : p->Jb;
-        while ((size_t)(bs * 2) * (bs * 2) * gbytes <= p->scratch_bytes && bs * 2 <= n_occ) bs *= 2;
+        while ((size_t)(bs * 2) * (bs * 2) * gbytes <= p->scratch_bytes && bs * 2 <= n_occ && (bs * 2) * (bs * 2) <= 65535) bs *= 2;
         for (int j0 = 0; j0 < n_occ; j0 += bs) {
             const int nj = (n_occ - j0 < bs) ? n_occ - j0 : bs;
             for (int i0 = 0; i0 <= j0; i0 += bs) {

@@ -175,3 +175,17 @@ def test_oversized_tile_is_clamped(cuda_device):
     cols = [0, 149, 299]
     ref = _oracle(cfg, phi, psi[cols].contiguous())
     assert _rel(out[cols].cpu().numpy(), ref) <= TOL
+
+
+def test_symmetric_blocks_stay_launchable(cuda_device):
+    """Psi = Phi with 512 orbitals on 16^3: the square block of the symmetric schedule must stop doubling before
+    block^2 pair-solves exceed what one launch can index."""
+    cfg = synth.Config("sym512", (10.26,) * 3, (16, 16, 16), 512, synth.KERNEL_COULOMB)
+    phi = synth.random_orbitals(cfg, 9, 512, cuda_device)
+    with binding.plan_for(cfg) as plan:
+        out = plan.apply(phi)
+        torch.cuda.synchronize()
+        assert plan.info()["last_symmetric"] == 1
+    cols = [0, 255, 511]
+    ref = _oracle(cfg, phi, cols=cols)
+    assert _rel(out[cols].cpu().numpy(), ref) <= TOL
