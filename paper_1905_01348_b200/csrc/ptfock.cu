@@ -371,12 +371,29 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     }
     // pair-scheduler tile
     int Ib = d.block_i > 0 ? d.block_i : 64;
-    // targets per wave: enough (target, x0) CTAs for ~7 full rounds of the 148 SMs in passes A and C
-    int Jb = d.block_j > 0 ? d.block_j : (1024 / d.n[0] > 8 ? 1024 / d.n[0] : 8);
+    // targets per wave: passes A and C launch Jb * n0 one-per-SM CTAs; aim at ~7 rounds of the SMs and, if the last
+    // round would be badly filled (n0 = 120: 960 CTAs = 6.5 rounds), take the next Jb (a divisor of max_targets if
+    // there is one) that fills whole rounds
+    int Jb = d.block_j;
+    if (Jb <= 0) {
+        const int sms = prop.multiProcessorCount, base = (1024 / d.n[0] > 8 ? 1024 / d.n[0] : 8);
+        auto eff = [&](int c) {
+            const long long ctas = (long long)c * d.n[0], rounds = (ctas + sms - 1) / sms;
+            return (double)ctas / (double)(rounds * sms);
+        };
+        Jb = base;
+        for (int pass = 0; pass < 2 && Jb == base; ++pass) {
+            double best = eff(base) + 0.02;
+            for (int c = base + 1; c <= 2 * base && c <= d.max_targets; ++c) {
+                if (pass == 0 && d.max_targets % c) continue;
+                if (eff(c) > best) { best = eff(c); Jb = c; }
+            }
+        }
+    }
     if (Ib > d.n_occ) Ib = d.n_occ;
     if (Jb > d.max_targets) Jb = d.max_targets;
     const size_t pair_bytes = sizeof(cd) * (size_t)p->N;
-    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)6 << 30);
+    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)12 << 30);
     while ((long long)Ib * Jb > 65535 && Ib > 1) Ib = (Ib + 1) / 2;     // pass B puts the wave's pairs on gridDim.y
     while ((long long)Ib * Jb > 65535 && Jb > 1) Jb = (Jb + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
