@@ -64,6 +64,14 @@ PTF_DEV void tile_load(cd (&u)[R * C], const cd *p) {
 #pragma unroll
         for (int c = 0; c < C; ++c) u[r * C + c] = p[r * SR + c * SC];
 }
+// same, from global memory past L1 (streamed once: keep the L1/shared SRAM for the tiles)
+template <int R, int C, int SR, int SC>
+PTF_DEV void tile_load_cg(cd (&u)[R * C], const cd *p) {
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int c = 0; c < C; ++c) u[r * C + c] = __ldcg(reinterpret_cast<const double2 *>(p + r * SR + c * SC));
+}
 template <int R, int C, int SR, int SC>
 PTF_DEV void tile_store(const cd (&u)[R * C], cd *p) {
 #pragma unroll
@@ -490,7 +498,7 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
             if (c + 1 < C1) {
 #pragma unroll
                 for (int r = 0; r < R1; ++r)
-                    f[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2 + (c + 1) * B2));
+                    f[r] = __ldcg(reinterpret_cast<const double2 *>(phi + r * B1 * N2 + (c + 1) * B2));
             }
         }
     };
@@ -513,7 +521,7 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
         cd fq[S::Q ? R1 : 1];
         if (S::Q && act1) {     // first column block of phi_i: in flight during stage 2'
 #pragma unroll
-            for (int r = 0; r < R1; ++r) fq[r] = __ldg(reinterpret_cast<const double2 *>(phi + r * B1 * N2));
+            for (int r = 0; r < R1; ++r) fq[r] = __ldcg(reinterpret_cast<const double2 *>(phi + r * B1 * N2));
         }
         stage2i(T);
         __syncthreads();
@@ -529,7 +537,7 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
                 tile_load<R1, C1, A::RA, A::COLB>(u, T + base1);
                 DFT<B2, true>::run(w);
                 tile_store<1, B2, 0, A::COL1>(w, p3);
-                tile_load<R1, C1, B1 * N2, B2>(f, phi);      // phi_i (L2-prefetched): lands during the next DFT
+                tile_load_cg<R1, C1, B1 * N2, B2>(f, phi);      // phi_i (L2-prefetched): lands during the next DFT
                 dft_over_r<R1, C1, true>(u);
                 if (g.conj_w) {
 #pragma unroll
@@ -546,7 +554,7 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
                 }
             } else {
                 cd f[R1 * C1];
-                tile_load<R1, C1, B1 * N2, B2>(f, phi);
+                tile_load_cg<R1, C1, B1 * N2, B2>(f, phi);
                 stage3i_p(T, f);
                 if (more) {
                     mbar_wait(&bars[(it + 1) % NBUF], ((it + 1) / NBUF) & 1);
