@@ -62,7 +62,14 @@ typedef struct {
     int32_t block_i;          /* pair-scheduler tile: orbitals i per wave (0 = library chooses)            */
     int32_t block_j;          /* pair-scheduler tile: targets j per wave  (0 = library chooses)            */
     uint64_t workspace_bytes; /* upper bound for the pair-density scratch (0 = library chooses)            */
+    uint32_t flags;           /* PTFOCK_FLAG_* (0 = library chooses the kernels)                            */
 } ptfock_desc;
+
+enum {
+    /* use the three-stage slab passes (slabx.cuh) even where the two-stage passes (pass8.cuh) exist: same
+     * results, kept for A/B timing and as a second implementation the tests compare with the oracle */
+    PTFOCK_FLAG_THREE_STAGE_SLABS = 1u
+};
 
 /* Builds the plan: v(G) table (with -alpha/N folded in, stored in the kernels' digit-permuted
  * frequency order), twiddle tables, scratch for one wave of pair densities.  *out is written only
@@ -125,6 +132,12 @@ int ptfock_get_profile(ptfock_plan *plan, double ms[3], int64_t launches[3], int
  * MEASURED_PEAKS.json records no FP64 number): runs a register-resident DFMA loop on `device` (legacy default
  * stream, synchronous, ~50 ms) and writes the best sustained rate in TFLOP/s (2 flops per DFMA) to HOST memory. */
 int ptfock_measure_dfma_peak(int32_t device, double *tflops_host);
+
+/* Measurement aid for the scratch-residency question (SURVEY.md 8(d) "a third roof to watch"):
+ * copies `bytes` bytes device-to-device `reps` times back to back with a plain 128-bit grid-stride kernel and
+ * writes the best read+write rate in GB/s to HOST memory.  A working set (2 * bytes) well under the L2 size
+ * measures the L2 copy bandwidth, one well above it the HBM copy bandwidth.  Synchronous, legacy default stream. */
+int ptfock_measure_copy_bandwidth(int32_t device, uint64_t bytes, int32_t reps, double *gbs_host);
 
 #ifdef __cplusplus
 }

@@ -17,10 +17,11 @@ SRC_DIR = os.path.join(_HERE, "csrc")
 
 KERNEL_COULOMB = 0
 KERNEL_HSE = 1
+FLAG_THREE_STAGE_SLABS = 1
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
-           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak"]
+           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_copy_bandwidth"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -36,7 +37,7 @@ class Desc(ctypes.Structure):
     _fields_ = [("cell", ctypes.c_double * 9), ("n", ctypes.c_int32 * 3), ("n_occ", ctypes.c_int32),
                 ("max_targets", ctypes.c_int32), ("kernel", ctypes.c_int32), ("omega", ctypes.c_double),
                 ("alpha", ctypes.c_double), ("device", ctypes.c_int32), ("block_i", ctypes.c_int32),
-                ("block_j", ctypes.c_int32), ("workspace_bytes", ctypes.c_uint64)]
+                ("block_j", ctypes.c_int32), ("workspace_bytes", ctypes.c_uint64), ("flags", ctypes.c_uint32)]
 
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
@@ -77,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.ptfock_set_profiling.argtypes = [vp, i32]
         L.ptfock_get_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64), i32]
         L.ptfock_measure_dfma_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double)]
+        L.ptfock_measure_copy_bandwidth.argtypes = [i32, ctypes.c_uint64, i32, ctypes.POINTER(ctypes.c_double)]
         for name in EXPORTS:
             if name != "ptfock_strerror":
                 getattr(L, name).restype = ctypes.c_int
@@ -123,7 +125,7 @@ class Plan:
 
     def __init__(self, cell, n, n_occ: int, max_targets: int | None = None, kernel: int = KERNEL_HSE,
                  omega: float = 0.106, alpha: float = 1.0, device: int = 0, block_i: int = 0, block_j: int = 0,
-                 workspace_bytes: int = 0):
+                 workspace_bytes: int = 0, flags: int = 0):
         d = Desc()
         cell = [float(x) for x in cell]
         if len(cell) != 9 or len(n) != 3:
@@ -134,6 +136,7 @@ class Plan:
         d.max_targets = int(n_occ if max_targets is None else max_targets)
         d.kernel, d.omega, d.alpha, d.device = int(kernel), float(omega), float(alpha), int(device)
         d.block_i, d.block_j, d.workspace_bytes = int(block_i), int(block_j), int(workspace_bytes)
+        d.flags = int(flags)
         self._h = ctypes.c_void_p(0)
         self.n = tuple(int(x) for x in n)
         self.N = self.n[0] * self.n[1] * self.n[2]
@@ -236,6 +239,14 @@ def measure_fp64_peak(device: int = 0) -> float:
     """Sustained DFMA rate of the device in TFLOP/s (ptfock_measure_dfma_peak)."""
     v = ctypes.c_double(0.0)
     _check(lib().ptfock_measure_dfma_peak(int(device), ctypes.byref(v)), "ptfock_measure_dfma_peak")
+    return v.value
+
+
+def measure_copy_bandwidth(nbytes: int, reps: int = 20, device: int = 0) -> float:
+    """Device-to-device copy rate in GB/s (read + write) for a source of ``nbytes`` (ptfock_measure_copy_bandwidth)."""
+    v = ctypes.c_double(0.0)
+    _check(lib().ptfock_measure_copy_bandwidth(int(device), int(nbytes), int(reps), ctypes.byref(v)),
+           "ptfock_measure_copy_bandwidth")
     return v.value
 
 

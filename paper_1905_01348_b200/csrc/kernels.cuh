@@ -328,6 +328,18 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters,
     if (r == 123.456) sink[0] = r;          // never true: keeps the loop alive
 }
 
+// ---- copy bandwidth (measurement aid: L2-resident vs HBM-resident working sets) ------------------
+// dst[k] = src[k] over n 16-byte elements, grid-stride, 4 independent 128-bit loads in flight per thread.
+__global__ void __launch_bounds__(256) copy_bw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long n) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; k + 3 * stride < n; k += 4 * stride) {
+        const double2 a = src[k], b = src[k + stride], c = src[k + 2 * stride], d = src[k + 3 * stride];
+        dst[k] = a; dst[k + stride] = b; dst[k + 2 * stride] = c; dst[k + 3 * stride] = d;
+    }
+    for (; k < n; k += stride) dst[k] = src[k];
+}
+
 // ---- helpers --------------------------------------------------------------------------------------
 // partial[b] = sum over the block's share of conj(psi) * vx
 __global__ void __launch_bounds__(256) dot_partial(const cd *psi, const cd *vx, long long n, double2 *partial) {

@@ -6,6 +6,7 @@
 #include "slab2.cuh"
 #include "slabx.cuh"
 #include "pencil_tma.cuh"
+#include "pass8.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -150,6 +151,36 @@ const PencilEntry kPencils[] = { PENCIL_REG(16), PENCIL_REG(32), PENCIL_REG(48),
 #undef PENCIL_REG
 #undef PENCIL
 
+// ---- 8 + 10 + 8 bit split (pass8.cuh) ---------------------------------------------------------------------------
+struct P8Entry {
+    int n0, n1, n2, a0, a1, a2;                 // k0 = k0a + a0*k0b, k1 = k1a + a1*k1b, k2 = k2a + a2*k2b
+    int nq, rq, p, rows, qpts, npos, ntb, minb_ac;
+    void (*fwd)(const SlabArgs &, dim3, cudaStream_t);
+    void (*inv)(const SlabArgs &, dim3, cudaStream_t);
+    void (*mid)(const CUtensorMap &, const P8MidArgs &, int pairs, cudaStream_t);
+    cudaError_t (*prepare)();
+};
+template <class S> void launch_p8_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) { p8_fwd<S><<<grid, S::NT, S::SMEM_A, st>>>(a); }
+template <class S> void launch_p8_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) { p8_inv_acc<S><<<grid, S::NT, S::SMEM_C, st>>>(a); }
+template <class S> void launch_p8_mid(const CUtensorMap &m, const P8MidArgs &a, int pairs, cudaStream_t st) {
+    p8_mid<S><<<dim3(S::NGRP, pairs), S::NTB, S::SMEM_B, st>>>(m, a);
+}
+template <class S> cudaError_t prepare_p8() {
+    cudaError_t e = cudaFuncSetAttribute(p8_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_A);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(p8_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_C);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(p8_mid<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_B);
+    // several small CTAs per SM: ask for the largest shared-memory carve-out
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(p8_fwd<S>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(p8_inv_acc<S>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(p8_mid<S>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    return e;
+}
+typedef P8<64, 64, 64, 4, 4, 2> P8_64;
+#define P8E(S) { S::N0, S::N1, S::N2, S::A0, S::A1, S::A2, S::NQ, S::RQ, S::P, S::ROWS, S::QPTS, S::NPOS, S::NTB, 6, \
+                 launch_p8_fwd<S>, launch_p8_inv<S>, launch_p8_mid<S>, prepare_p8<S> }
+const P8Entry kP8[] = { P8E(P8_64) };
+#undef P8E
+
 // position -> frequency index of the digit-permuted order the forward passes leave an axis in
 int freq_of_pos(int r1, int r2, int pos) {
     const int k1 = pos / r2, k2 = pos % r2;
@@ -202,6 +233,10 @@ struct ptfock_plan {
     int last_symmetric;
     CUtensorMap tmap;                   // pair scratch as [pairs*n0 rows][2*slab_pts doubles] (pass B, TMA variant)
     int use_tma;
+    // 8 + 10 + 8 bit split (pass8.cuh): own tensor map (128-byte swizzle) and v' table in pass B's register order
+    const struct P8Entry *p8;
+    CUtensorMap tmap8;
+    double2 *v8_dev;
     // optional per-pass device timing (ptfock_set_profiling): events bracket every launch
     int profiling;
     std::vector<cudaEvent_t> *ev_pool;
@@ -223,6 +258,7 @@ bool edge_ok(int n) {
 void free_plan(ptfock_plan *p) {
     if (!p) return;
     cudaFree(p->v_dev);
+    cudaFree(p->v8_dev);
     for (int d = 0; d < 3; ++d) cudaFree(p->tw_dev[d]);
     cudaFree(p->scratch);
     cudaFree(p->partials);
@@ -241,7 +277,7 @@ void free_plan(ptfock_plan *p) {
 
 // v'(pos0, pos1, pos2) = -alpha/N * v(|G|^2) in the permuted order; also reports whether v(-G) = v(G)
 // holds on the grid (needed by the pair-symmetric schedule; fails for skew cells at Nyquist planes).
-int build_vtable(const ptfock_desc &d, const SlabEntry &se, std::vector<double> &vperm, bool &even) {
+int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, std::vector<double> &vperm, bool &even) {
     const int n0 = d.n[0], n1 = d.n[1], n2 = d.n[2];
     const long long N = (long long)n0 * n1 * n2;
     const double *a = d.cell;
@@ -288,6 +324,25 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, std::vector<double> 
             }
     const double scale = -d.alpha / (double)N;
     vperm.resize((size_t)N);
+    if (p8) {
+        // pass8.cuh order: [tile group][m < 16][middle-stage thread t < ntb] pairs (k0b = 2m, 2m + 1), where
+        // t = ((k0a*nq + q)*p + pp)*rq + r, k1b = q*rq + r, slab position = group*p + pp = (k2b*a1 + k1a)*a2 + k2a
+        const int ngrp = p8->npos / p8->p;
+        for (int grp = 0; grp < ngrp; ++grp)
+            for (int m = 0; m < 16; ++m)
+                for (int t = 0; t < p8->ntb; ++t) {
+                    const int r = t % p8->rq, pp = (t / p8->rq) % p8->p, q = (t / (p8->rq * p8->p)) % p8->nq;
+                    const int k0a = t / (p8->rq * p8->p * p8->nq);
+                    const int pos = grp * p8->p + pp;
+                    const int k2a = pos % p8->a2, k1a = (pos / p8->a2) % p8->a1, k2b = pos / (p8->a2 * p8->a1);
+                    const int k1 = k1a + p8->a1 * (q * p8->rq + r), k2 = k2a + p8->a2 * k2b;
+                    for (int h = 0; h < 2; ++h) {
+                        const int k0 = k0a + p8->a0 * (2 * m + h);
+                        vperm[(((size_t)grp * 16 + m) * p8->ntb + t) * 2 + h] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
+                    }
+                }
+        return PTFOCK_OK;
+    }
     int p_r1, p_r2;
     pencil_split(n0, p_r1, p_r2);
     for (int p0 = 0; p0 < n0; ++p0) {
@@ -327,6 +382,9 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     for (const PencilEntry &e : kPencils) if (e.n0 == d.n[0]) pencil = &e;
     if (!slab || !pencil) return PTFOCK_ERR_UNSUPPORTED_GRID;
     if (det3(d.cell) == 0.0) return PTFOCK_ERR_INVALID_ARG;
+    const P8Entry *p8 = nullptr;
+    if (!(d.flags & PTFOCK_FLAG_THREE_STAGE_SLABS))
+        for (const P8Entry &e : kP8) if (e.n0 == d.n[0] && e.n1 == d.n[1] && e.n2 == d.n[2]) p8 = &e;
 
     int ndev = 0;
     CU(cudaGetDeviceCount(&ndev));
@@ -345,20 +403,27 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     p->volume = std::fabs(det3(d.cell));
     p->slab = slab;
     p->pencil = pencil;
+    p->p8 = p8;
 
     std::vector<double> vperm;
     bool even = false;
-    int rc = build_vtable(d, *slab, vperm, even);
+    int rc = build_vtable(d, *slab, p8, vperm, even);
     if (rc != PTFOCK_OK) { free_plan(p); return rc; }
     p->v_even = even;
 
 #define CUP(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_cuda = (int)e__; free_plan(p); \
         return (e__ == cudaErrorMemoryAllocation) ? PTFOCK_ERR_ALLOC : PTFOCK_ERR_CUDA; } } while (0)
 
-    CUP(slab->prepare());
-    CUP(pencil->prepare());
-    CUP(cudaMalloc(&p->v_dev, sizeof(double) * p->N));
-    CUP(cudaMemcpy(p->v_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
+    if (p8) {
+        CUP(p8->prepare());
+        CUP(cudaMalloc(&p->v8_dev, sizeof(double) * p->N));
+        CUP(cudaMemcpy(p->v8_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
+    } else {
+        CUP(slab->prepare());
+        CUP(pencil->prepare());
+        CUP(cudaMalloc(&p->v_dev, sizeof(double) * p->N));
+        CUP(cudaMemcpy(p->v_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
+    }
     for (int k = 0; k < 3; ++k) {
         const int n = d.n[k];
         std::vector<cd> tw((size_t)n);
@@ -405,26 +470,34 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     CUP(cudaMalloc(&p->scratch, p->scratch_bytes));
     p->use_tma = 0;
     {
-        const char *pk = std::getenv("PTFOCK_PENCIL");          // "legacy": the register-path pencil kernel (comparison runs)
-        if (pencil->run_tma && !(pk && std::strcmp(pk, "legacy") == 0)) {
-            typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                          const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                          CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-            void *fn = nullptr;
-            cudaDriverEntryPointQueryResult qres;
-            CUP(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
-            if (fn && qres == cudaDriverEntryPointSuccess) {
-                const cuuint64_t dims[2] = { (cuuint64_t)2 * p->slab_pts, (cuuint64_t)Ib * Jb * d.n[0] };
-                const cuuint64_t strides[1] = { (cuuint64_t)p->slab_pts * sizeof(cd) };
-                const cuuint32_t box[2] = { (cuuint32_t)(2 * pencil->tma_cw), (cuuint32_t)d.n[0] };
-                const cuuint32_t estr[2] = { 1, 1 };
-                CUresult r = ((encode_fn)fn)(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
-                                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-                if (r == CUDA_SUCCESS) {
-                    CUP(pencil->prepare_tma());
-                    p->use_tma = 1;
-                }
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CUP(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        const bool have = fn && qres == cudaDriverEntryPointSuccess;
+        const cuuint32_t estr[2] = { 1, 1 };
+        if (p8) {
+            // scratch as [pairs * nq * n0 rows][2 * qpts doubles]; box = 128 bytes x all (q, x0) rows of one pair
+            if (!have) { free_plan(p); return PTFOCK_ERR_CUDA; }
+            const cuuint64_t dims[2] = { (cuuint64_t)2 * p8->qpts, (cuuint64_t)Ib * Jb * p8->rows };
+            const cuuint64_t strides[1] = { (cuuint64_t)p8->qpts * sizeof(cd) };
+            const cuuint32_t box[2] = { (cuuint32_t)(2 * p8->p * p8->rq), (cuuint32_t)p8->rows };
+            CUresult r = ((encode_fn)fn)(&p->tmap8, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
+                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) { g_last_cuda = (int)r; free_plan(p); return PTFOCK_ERR_CUDA; }
+        } else if (pencil->run_tma && have) {
+            const cuuint64_t dims[2] = { (cuuint64_t)2 * p->slab_pts, (cuuint64_t)Ib * Jb * d.n[0] };
+            const cuuint64_t strides[1] = { (cuuint64_t)p->slab_pts * sizeof(cd) };
+            const cuuint32_t box[2] = { (cuuint32_t)(2 * pencil->tma_cw), (cuuint32_t)d.n[0] };
+            CUresult r = ((encode_fn)fn)(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
+                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r == CUDA_SUCCESS) {
+                CUP(pencil->prepare_tma());
+                p->use_tma = 1;
             }
         }
     }
@@ -512,9 +585,20 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
     // split the i loop over blockIdx.z until the grid has a few CTAs per SM
     int z = 1;
     const long long base = (long long)p->d.n[0] * nj;
-    while (z < ni && base * z < 148LL * 6) z *= 2;
+    while (z < ni && base * z * (p->p8 ? p->p8->nq : 1) < 148LL * (p->p8 ? 12 : 6)) z *= 2;
     if (z > ni) z = ni;
     mark(w, -1);
+    if (p->p8) {
+        p->p8->fwd(a, dim3(nj, p->d.n[0] * p->p8->nq, z), w.st);
+        mark(w, 0);
+        P8MidArgs b;
+        b.v = p->v8_dev; b.tw0 = p->tw_dev[0];
+        p->p8->mid(p->tmap8, b, ni * nj, w.st);
+        mark(w, 1);
+        w.launches += 2;
+        w.pairs += (long long)ni * nj;
+        return;
+    }
     p->slab->fwd(a, dim3(nj, p->d.n[0], z), w.st);
     mark(w, 0);
     if (p->use_tma) {
@@ -541,7 +625,8 @@ void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, in
     a.grid_pts = p->N; a.n0 = p->d.n[0];
     a.a0 = s0; a.na = ns; a.b0 = t0;
     a.stride_loop = stride_loop; a.stride_cta = stride_cta; a.conj_w = conj_w;
-    p->slab->inv(a, dim3(nt, p->d.n[0], 1), w.st);
+    if (p->p8) p->p8->inv(a, dim3(nt, p->d.n[0] * p->p8->nq, 1), w.st);
+    else p->slab->inv(a, dim3(nt, p->d.n[0], 1), w.st);
     mark(w, 2);
     w.launches += 1;
 }
@@ -783,6 +868,42 @@ extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
     cudaFree(sink);
     *tflops_host = best;
     return PTFOCK_OK;
+}
+
+extern "C" int ptfock_measure_copy_bandwidth(int32_t device, uint64_t bytes, int32_t reps, double *gbs_host) {
+    if (!gbs_host || bytes < 4096 || reps < 1) return PTFOCK_ERR_INVALID_ARG;
+    CU(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
+    const long long n = (long long)(bytes / sizeof(double2));
+    double2 *src = nullptr, *dst = nullptr;
+    if (cudaMalloc(&src, n * sizeof(double2)) != cudaSuccess) return PTFOCK_ERR_ALLOC;
+    if (cudaMalloc(&dst, n * sizeof(double2)) != cudaSuccess) { cudaFree(src); return PTFOCK_ERR_ALLOC; }
+    cudaMemset(src, 0, n * sizeof(double2));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int blocks = prop.multiProcessorCount * 8;
+    double best = 0.0;
+    int rc = PTFOCK_OK;
+    for (int rep = 0; rep < 5 && rc == PTFOCK_OK; ++rep) {          // the working set stays where the previous pass left it
+        cudaEventRecord(e0, 0);
+        for (int r = 0; r < reps; ++r) copy_bw_kernel<<<blocks, 256>>>(src, dst, n);
+        cudaEventRecord(e1, 0);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; rc = PTFOCK_ERR_CUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double gbs = 2.0 * (double)n * sizeof(double2) * reps / (ms * 1e-3) / 1e9;
+        if (rep >= 1 && gbs > best) best = gbs;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(src);
+    cudaFree(dst);
+    *gbs_host = best;
+    return rc;
 }
 
 extern "C" int ptfock_set_profiling(ptfock_plan *plan, int32_t on) {
