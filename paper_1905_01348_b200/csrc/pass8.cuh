@@ -23,9 +23,6 @@
 #include "kernels.cuh"
 #include "tma.cuh"
 
-#ifndef P8_VMODE
-#define P8_VMODE 2
-#endif
 #ifndef P8_A_PREF
 #define P8_A_PREF 0          // 1: pass A prefetches the next phi_i through registers (255 registers, 4 CTAs per SM)
 #endif
@@ -34,12 +31,6 @@
 #endif
 #ifndef P8_C_L2PF
 #define P8_C_L2PF 2          // pass C: L2 prefetch distance (iterations) for the pair-density rows, 0 = off
-#endif
-#ifndef P8_SKEL_B
-#define P8_SKEL_B 0          // timing experiments only: 1 = butterflies compiled out, 2 = tile load + store only
-#endif
-#ifndef P8_MAXREG_B
-#define P8_MAXREG_B 168
 #endif
 
 namespace ptfock {
@@ -57,11 +48,13 @@ struct P8 {
     static_assert(NT == NT2 && NT == 64, "one task per thread in both stages");
     static constexpr int PW = B2 + 1;                       // exchange tile pitch (elements): conflict free both ways
     static constexpr int WORK = NT2 * PW;
-    static constexpr int SMEM_A = 2 * WORK * 16;            // two exchange tiles: one CTA barrier per orbital
-    static constexpr int SMEM_C = SMEM_A + (A1 - 1 + A2 - 1) * NT * 16;       // + per-thread twiddles
     static constexpr int QPTS = A1 * RQ * N2;               // points of one (slab, q) row of the scratch
     static constexpr int NPOS = A1 * A2 * B2;               // slab positions (k2b, k1a, k2a) per row
-    static constexpr int MAXREG_A = P8_A_PREF ? 255 : 168, MAXREG_C = P8_C_PREF ? 255 : 192;    // 6 / 4 CTAs per SM
+    static constexpr int NBUF_A = 2;                        // pass A: ring of landed phi_i quarter slabs
+    static constexpr int SMEM_A = NBUF_A * QPTS * 16 + 64;
+    static constexpr int NBUF_C = 3;                        // pass C: ring of landed pair-density rows
+    static constexpr int SMEM_C = NBUF_C * QPTS * 16 + 64;
+    static constexpr int MAXREG_A = 168, MAXREG_C = 255;    // 6 / 4 CTAs per SM
     // pass B
     static constexpr int P = 2;                             // slab positions per tile: rows of P*RQ*16 = 128 bytes
     static constexpr int ROWS = NQ * N0;                    // tile rows (q, x0)
@@ -69,8 +62,10 @@ struct P8 {
     static constexpr int TILE_B = ROWS * P * RQ * 16;       // 32 KB
     static constexpr int NTB = 32 * P;                      // 64 threads
     static_assert(A0 * NQ * P * RQ == NTB, "middle-stage tasks");
-    static constexpr int SMEM_B = TILE_B + 16;              // + mbarrier
-    static constexpr int MINB_B = 6;
+    static constexpr int GB = 3;                            // tiles (64-thread groups) per CTA, sharing one copy of v'
+    static constexpr int V_BYTES = ROWS * P * RQ * 8;       // 16 KB
+    static constexpr int SMEM_B = GB * TILE_B + V_BYTES + 64;   // + mbarriers: 2 CTAs (6 tiles) per SM
+    static constexpr int MAXREG_B = 168;                    // 12 warps per SM
     static constexpr int NGRP = NPOS / P;                   // tiles per pair
 };
 
@@ -165,13 +160,17 @@ PTF_DEV cd ldcg_v(const cd *p) {
 }
 
 // grid = (targets in the wave, N0 * NQ, chunks of the i loop); 64 threads.  Registers: psi_j (16 points = 64 registers)
-// + the working tile (64) + twiddles; phi_i is NOT prefetched through registers -- the other CTAs of the SM (MINB_A of
-// them, out of phase) cover its latency.
+// + the working tile (64) + twiddles.  phi_i's quarter slab (RQ rows of every a1 chunk: A1 runs of 4 KB) arrives by
+// 1-D bulk async copies (TMA) in a ring of NBUF_A shared-memory buffers, one iteration ahead and without holding
+// registers; both stages work IN PLACE in the landed buffer, exchanging through an XOR swizzle (slot (t2, b2) at
+// t2*B2 + (b2 ^ (t2 & 7))), conflict free both ways; results leave from registers in 1 KB runs.
 template <class S>
 __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
-    constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ, PW = S::PW;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cd *work = reinterpret_cast<cd *>(smem_raw);
+    constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ;
+    constexpr int NBUF = S::NBUF_A, CH = RQ * N2;        // one a1 chunk: RQ contiguous rows
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    cd *ring = reinterpret_cast<cd *>(smem_raw);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
     const int tid = threadIdx.x;
     const int jj = blockIdx.x, x0 = blockIdx.y / S::NQ, q = blockIdx.y % S::NQ;
     const int per = (g.na + gridDim.z - 1) / gridDim.z;
@@ -181,6 +180,27 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     // stage-1 task (r, b2): the 4 x 4 points (a1, a2) at x1 = a1*B1 + b1, x2 = a2*B2 + b2
     const int b2 = tid % B2, r = tid / B2, b1 = q * RQ + r;
     const long long off1 = (long long)x0 * (N1 * N2) + b1 * N2 + b2;
+    // chunk a1 of the quarter slab of orbital it: phi0 + it*grid_pts + a1*B1*N2
+    const cd *phi0 = g.a + (long long)(g.a0 + ii_beg) * g.grid_pts + (long long)x0 * (N1 * N2) + (q * RQ) * N2;
+    auto issue = [&](int it) {          // warp 0: lanes 0 .. A1-1 copy one chunk each
+        const int buf = it % NBUF;
+        if (tid == 0) mbar_expect_tx(&bars[buf], S::QPTS * 16u);
+        __syncwarp();
+        if (tid < A1)
+            bulk_g2s(ring + buf * S::QPTS + tid * CH, phi0 + (long long)it * g.grid_pts + (long long)tid * (B1 * N2), CH * 16u, &bars[buf]);
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < NBUF; ++k) mbar_init(&bars[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+    if (tid < 32) {
+#pragma unroll
+        for (int k = 0; k < NBUF - 1; ++k)
+            if (k < n_it) issue(k);
+    }
     cd pj[A1 * A2];
     {
         const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + off1;
@@ -194,40 +214,24 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     for (int k = 1; k < A1; ++k) tw1[k - 1] = g.tw1[b1 * k];          // w_N1^(b1 k1a)
 #pragma unroll
     for (int k = 1; k < A2; ++k) tw2[k - 1] = g.tw2[b2 * k];          // w_N2^(b2 k2a)
-    const cd *phi = g.a + (long long)(g.a0 + ii_beg) * g.grid_pts + off1;
-    const int st1 = r * PW + b2;                                       // + (k1a*A2 + k2a) * RQ * PW
+    const int ld1 = r * N2 + b2;                                       // + a1*CH + a2*B2
     const long long pair0 = (long long)ii_beg * g.stride_loop + (long long)jj * g.stride_cta;
     cd *dst = g.scratch + ((pair0 * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS + tid;
     const long long dst_step = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
-#if P8_A_PREF
-    cd f[A1 * A2];
-#pragma unroll
-    for (int a1 = 0; a1 < A1; ++a1)
-#pragma unroll
-        for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
-#endif
 #pragma unroll 1
     for (int it = 0; it < n_it; ++it) {
+        cd *T = ring + (it % NBUF) * S::QPTS;
+        mbar_wait(&bars[it % NBUF], (it / NBUF) & 1);
         cd u[A1 * A2];
-#if P8_A_PREF
-#pragma unroll
-        for (int k = 0; k < A1 * A2; ++k) u[k] = cmulc(pj[k], f[k]);  // psi_j conj(phi_i)
-        phi += g.grid_pts;
-        if (it + 1 < n_it) {
-#pragma unroll
-            for (int a1 = 0; a1 < A1; ++a1)
-#pragma unroll
-                for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
-        }
-#else
 #pragma unroll
         for (int a1 = 0; a1 < A1; ++a1)
 #pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) u[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
-        phi += g.grid_pts;
+            for (int a2 = 0; a2 < A2; ++a2) u[a1 * A2 + a2] = T[ld1 + a1 * CH + a2 * B2];
+        fence_proxy_async();
+        __syncthreads();                                // phi_i read; the buffer of iteration it - 1 is free
+        if (tid < 32 && it + NBUF - 1 < n_it) issue(it + NBUF - 1);
 #pragma unroll
         for (int k = 0; k < A1 * A2; ++k) u[k] = cmulc(pj[k], u[k]);  // psi_j conj(phi_i)
-#endif
         dft_rows<A1, A2, false>(u);
 #pragma unroll
         for (int k1 = 1; k1 < A1; ++k1)
@@ -238,14 +242,14 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
         for (int k2 = 1; k2 < A2; ++k2)
 #pragma unroll
             for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmul(u[k1 * A2 + k2], tw2[k2 - 1]);
-        cd *W = work + (it & 1) * S::WORK;
+        // value (k1a, k2a) of this thread belongs to stage-2 task t2 = (k1a*A2 + k2a)*RQ + r, index b2
 #pragma unroll
-        for (int k = 0; k < A1 * A2; ++k) W[st1 + k * (RQ * PW)] = u[k];
+        for (int k = 0; k < A1 * A2; ++k) T[(k * RQ + r) * B2 + (b2 ^ ((k * RQ + r) & 7))] = u[k];
         __syncthreads();
-        // stage 2: task tid = (k1a*A2 + k2a)*RQ + r, DFT over b2; output k2b at k2b*NT2 + tid of the scratch row
+        // stage 2: task tid, DFT over b2; output k2b at k2b*NT2 + tid of the scratch row
         cd w[B2];
 #pragma unroll
-        for (int b = 0; b < B2; ++b) w[b] = W[tid * PW + b];
+        for (int b = 0; b < B2; ++b) w[b] = T[tid * B2 + (b ^ (tid & 7))];
         DFT<B2, false>::run(w);
 #pragma unroll
         for (int m = 0; m < B2; ++m) dst[m * S::NT2] = w[m];
@@ -255,109 +259,106 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
 
 // ---- pass C ---------------------------------------------------------------------------------------------------
 // grid = (targets, N0 * NQ): out[b0+tt] += sum_ss a[a0+ss] * W[ss*stride_loop + tt*stride_cta]   (W or conj(W)).
-// Registers: the accumulators (64) + the working tile (64) + phi_i two columns at a time (32); the twiddles are re-read
-// from shared memory every iteration.
+// The pair-density rows (16 KB, contiguous) arrive by 1-D bulk async copies (TMA) in a ring of NBUF_C shared-memory
+// buffers, two iterations ahead and without holding registers: under load a global load takes several microseconds,
+// so an SM needs ~100 KB of reads in flight to keep HBM busy.  Both stages work IN PLACE in the landed buffer; the
+// exchange between them is an XOR swizzle (slot (b2, t2) at b2*NT2 + (t2 ^ (b2 & 7))), conflict free both ways.
+// phi_i is prefetched one iteration ahead through registers (16 points), accumulators in registers (16 points).
 template <class S>
 __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
-    constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ, PW = S::PW;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cd *work = reinterpret_cast<cd *>(smem_raw);
-    cd *tws = work + 2 * S::WORK;                  // [k-1][tid]: w_N1^(b1 k) for k < A1, then w_N2^(b2 k) for k < A2
+    constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ;
+    constexpr int NBUF = S::NBUF_C, NT2 = S::NT2;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    cd *ring = reinterpret_cast<cd *>(smem_raw);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
     const int tid = threadIdx.x;
     const int tt = blockIdx.x, x0 = blockIdx.y / S::NQ, q = blockIdx.y % S::NQ;
     const int n_it = g.na;
     if (n_it <= 0) return;
     const int b2 = tid % B2, r = tid / B2, b1 = q * RQ + r;
     const long long off1 = (long long)x0 * (N1 * N2) + b1 * N2 + b2;
+    const long long pair_stride = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
+    const cd *src = g.scratch + (((long long)tt * g.stride_cta * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS;
+    if (tid == 0) {
 #pragma unroll
-    for (int k = 1; k < A1; ++k) tws[(k - 1) * S::NT + tid] = g.tw1[b1 * k];
+        for (int k = 0; k < NBUF; ++k) mbar_init(&bars[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
 #pragma unroll
-    for (int k = 1; k < A2; ++k) tws[(A1 - 1 + k - 1) * S::NT + tid] = g.tw2[b2 * k];
+        for (int k = 0; k < NBUF - 1; ++k)
+            if (k < n_it) {
+                mbar_expect_tx(&bars[k], S::QPTS * 16u);
+                bulk_g2s(ring + k * S::QPTS, src + (long long)k * pair_stride, S::QPTS * 16u, &bars[k]);
+            }
+    }
+    cd tw1[A1 - 1], tw2[A2 - 1];
+#pragma unroll
+    for (int k = 1; k < A1; ++k) tw1[k - 1] = g.tw1[b1 * k];
+#pragma unroll
+    for (int k = 1; k < A2; ++k) tw2[k - 1] = g.tw2[b2 * k];
     cd acc[A1 * A2];
 #pragma unroll
     for (int k = 0; k < A1 * A2; ++k) acc[k] = make_double2(0.0, 0.0);
-    const long long pair_stride = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
-    const cd *src = g.scratch + (((long long)tt * g.stride_cta * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS + tid;
     const cd *phi = g.a + (long long)g.a0 * g.grid_pts + off1;
-    const int st1 = r * PW + b2;
+    cd f[A1 * A2];
+#pragma unroll
+    for (int a1 = 0; a1 < A1; ++a1)
+#pragma unroll
+        for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
     const bool cw = g.conj_w != 0;
-#if P8_C_L2PF
-    if (tid == 0) {
-#pragma unroll
-        for (int d = 1; d < P8_C_L2PF; ++d)
-            if (d < n_it) l2_prefetch_bulk(src - tid + (long long)d * pair_stride, S::QPTS * 16u);
-    }
-#endif
-#if P8_C_PREF
-    cd w[B2];
-#pragma unroll
-    for (int m = 0; m < B2; ++m) w[m] = ldcg_v(src + m * S::NT2);
-#endif
+    __syncthreads();                                    // mbarrier inits visible
 #pragma unroll 1
     for (int it = 0; it < n_it; ++it) {
-        cd *W = work + (it & 1) * S::WORK;
-#if P8_C_L2PF
-        if (tid == 0 && it + P8_C_L2PF < n_it) l2_prefetch_bulk(src + (long long)P8_C_L2PF * pair_stride, S::QPTS * 16u);
-#endif
-        {
-            // stage 1': inverse DFT over k2b of task tid = (k1a*A2 + k2a)*RQ + r
-#if !P8_C_PREF
-            cd w[B2];
+        cd *T = ring + (it % NBUF) * S::QPTS;
+        mbar_wait(&bars[it % NBUF], (it / NBUF) & 1);
+        cd w[B2];
 #pragma unroll
-            for (int m = 0; m < B2; ++m) w[m] = ldcg_v(src + m * S::NT2);
-#endif
-            src += pair_stride;
-            DFT<B2, true>::run(w);
-#pragma unroll
-            for (int b = 0; b < B2; ++b) W[tid * PW + b] = w[b];
-#if P8_C_PREF
-            if (it + 1 < n_it) {
-#pragma unroll
-                for (int m = 0; m < B2; ++m) w[m] = ldcg_v(src + m * S::NT2);
-            }
-#endif
+        for (int m = 0; m < B2; ++m) w[m] = T[m * NT2 + tid];
+        fence_proxy_async();
+        __syncthreads();                                // row read; the buffer of iteration it - 1 is free
+        if (tid == 0 && it + NBUF - 1 < n_it) {
+            const int nx = it + NBUF - 1;
+            mbar_expect_tx(&bars[nx % NBUF], S::QPTS * 16u);
+            bulk_g2s(ring + (nx % NBUF) * S::QPTS, src + (long long)nx * pair_stride, S::QPTS * 16u, &bars[nx % NBUF]);
         }
+        // stage 1': inverse DFT over k2b of task tid = (k1a*A2 + k2a)*RQ + r, back in place (swizzled)
+        DFT<B2, true>::run(w);
+#pragma unroll
+        for (int b = 0; b < B2; ++b) T[b * NT2 + (tid ^ (b & 7))] = w[b];
         __syncthreads();
         cd u[A1 * A2];
 #pragma unroll
-        for (int k = 0; k < A1 * A2; ++k) u[k] = W[st1 + k * (RQ * PW)];
-        cd f[2][A1];                                    // phi_i, columns a2 and a2 + 1 in flight
+        for (int k = 0; k < A1 * A2; ++k) u[k] = T[b2 * NT2 + ((k * RQ + r) ^ (b2 & 7))];
 #pragma unroll
-        for (int c = 0; c < 2 && c < A2; ++c)
+        for (int k2 = 1; k2 < A2; ++k2)
 #pragma unroll
-            for (int a1 = 0; a1 < A1; ++a1) f[c][a1] = ldcg_v(phi + a1 * (B1 * N2) + c * B2);
-#pragma unroll
-        for (int k2 = 1; k2 < A2; ++k2) {
-            const cd t2 = tws[(A1 - 1 + k2 - 1) * S::NT + tid];
-#pragma unroll
-            for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmulc(u[k1 * A2 + k2], t2);
-        }
+            for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmulc(u[k1 * A2 + k2], tw2[k2 - 1]);
         dft_cols<A1, A2, true>(u);
 #pragma unroll
-        for (int k1 = 1; k1 < A1; ++k1) {
-            const cd t1 = tws[(k1 - 1) * S::NT + tid];
+        for (int k1 = 1; k1 < A1; ++k1)
 #pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) u[k1 * A2 + a2] = cmulc(u[k1 * A2 + a2], t1);
-        }
+            for (int a2 = 0; a2 < A2; ++a2) u[k1 * A2 + a2] = cmulc(u[k1 * A2 + a2], tw1[k1 - 1]);
+        dft_rows<A1, A2, true>(u);
+        if (cw) {
 #pragma unroll
-        for (int a2 = 0; a2 < A2; ++a2) {
-            cd t[A1];
-#pragma unroll
-            for (int k1 = 0; k1 < A1; ++k1) t[k1] = u[k1 * A2 + a2];
-            DFT<A1, true>::run(t);
-#pragma unroll
-            for (int a1 = 0; a1 < A1; ++a1) {
-                const cd fv = f[a2 & 1][a1];
-                const cd pr = cw ? cmulc(fv, t[a1]) : cmul(fv, t[a1]);
-                acc[a1 * A2 + a2].x += pr.x;
-                acc[a1 * A2 + a2].y += pr.y;
+            for (int k = 0; k < A1 * A2; ++k) {
+                const cd pr = cmulc(f[k], u[k]);
+                acc[k].x += pr.x; acc[k].y += pr.y;
             }
-            if (a2 + 2 < A2) {
+        } else {
 #pragma unroll
-                for (int a1 = 0; a1 < A1; ++a1) f[a2 & 1][a1] = ldcg_v(phi + a1 * (B1 * N2) + (a2 + 2) * B2);
+            for (int k = 0; k < A1 * A2; ++k) {
+                const cd pr = cmul(f[k], u[k]);
+                acc[k].x += pr.x; acc[k].y += pr.y;
             }
         }
         phi += g.grid_pts;
+        if (it + 1 < n_it) {                            // next phi_i: on its way during the next iteration's first half
+#pragma unroll
+            for (int a1 = 0; a1 < A1; ++a1)
+#pragma unroll
+                for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
+        }
     }
     cd *o = g.out + (long long)(g.b0 + tt) * g.grid_pts + off1;
 #pragma unroll
@@ -375,6 +376,7 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
 struct P8MidArgs {
     const double2 *v;    // [tile group][16][64 threads]: the middle-stage thread's v' values (k0b = 2m, 2m + 1)
     const cd *tw0;       // exp(-2 pi i t / N0)
+    int n_pairs;         // pairs in the wave
 };
 
 PTF_DEV void tensor_g2s_2d_sw(void *dst_smem, const CUtensorMap *map, int c0, int c1, unsigned long long *bar) {
@@ -386,42 +388,40 @@ PTF_DEV void tensor_s2g_2d_sw(const CUtensorMap *map, int c0, int c1, const void
                  ::"l"(map), "r"(c0), "r"(c1), "r"(smem_u32(src_smem)) : "memory");
 }
 
-// grid = (NGRP tiles per pair, pairs); the tensor map views the scratch as [pairs*NQ*N0 rows][2*QPTS doubles] with
-// the 128-byte swizzle: element e of row R sits at (R*8 + (e ^ (R & 7))) * 16 bytes of the tile.
+// grid = (NGRP tile positions, ceil(pairs / GB)); a CTA is GB independent groups of 64 threads, one tile each (the same
+// tile position grp of GB consecutive pairs), sharing ONE copy of the position's v' values in shared memory, brought
+// in by a bulk async copy next to the tiles.  Why not a global load in the middle stage: an L2 hit issued while the
+// SM has tile loads outstanding queues behind them and costs a DRAM round trip (measured: 0.76 of the HBM peak with
+// the loads, 0.98 with the same arithmetic and no loads); why not registers: 64 more live registers halve the
+// CTAs per SM (0.83).  Groups synchronise among themselves with named barriers only.
+// The tensor map views the scratch as [pairs*NQ*N0 rows][2*QPTS doubles] with the 128-byte swizzle: element e of row R
+// sits at (R*8 + (e ^ (R & 7))) * 16 bytes of the tile.
 template <class S>
-__global__ void __maxnreg__(P8_MAXREG_B) p8_mid(const __grid_constant__ CUtensorMap map, const P8MidArgs g) {
-    constexpr int N0 = S::N0, A0 = S::A0, B1 = S::B1, RQ = S::RQ, NQ = S::NQ, P = S::P;
-    // the 128-byte swizzle pattern repeats every 1 KB: the tile must start on a 1 KB boundary of the shared window
+__global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensorMap map, const P8MidArgs g) {
+    constexpr int N0 = S::N0, A0 = S::A0, B1 = S::B1, RQ = S::RQ, NQ = S::NQ, P = S::P, GB = S::GB;
+    // the 128-byte swizzle pattern repeats every 1 KB: the tiles must start on 1 KB boundaries of the shared window
     extern __shared__ __align__(1024) unsigned char smem_b[];
-    cd *s = reinterpret_cast<cd *>(smem_b);
-    unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_b + S::TILE_B);
+    const double2 *vs = reinterpret_cast<const double2 *>(smem_b + GB * S::TILE_B);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_b + GB * S::TILE_B + S::V_BYTES);
     if (smem_u32(smem_b) & 1023u) __trap();
-    const int tid = threadIdx.x;
-    const int grp = blockIdx.x, row0 = blockIdx.y * S::ROWS;
-    if (tid == 0) {
-        mbar_init(bar, 1);
+    const int grp_pos = blockIdx.x;
+    const int gi = threadIdx.x / S::NTB, tid = threadIdx.x % S::NTB;       // group, thread in group
+    const int pair = blockIdx.y * GB + gi;
+    cd *s = reinterpret_cast<cd *>(smem_b + gi * S::TILE_B);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k <= GB; ++k) mbar_init(&bars[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
-        mbar_expect_tx(bar, S::TILE_B);
-        tensor_g2s_2d_sw(s, &map, grp * (P * RQ * 2), row0, bar);
+        mbar_expect_tx(&bars[GB], S::V_BYTES);
+        bulk_g2s(smem_b + GB * S::TILE_B, g.v + (long long)grp_pos * (S::V_BYTES / 16), S::V_BYTES, &bars[GB]);
+#pragma unroll
+        for (int k = 0; k < GB; ++k)
+            if (blockIdx.y * GB + k < g.n_pairs) {
+                mbar_expect_tx(&bars[k], S::TILE_B);
+                tensor_g2s_2d_sw(smem_b + k * S::TILE_B, &map, grp_pos * (P * RQ * 2), (blockIdx.y * GB + k) * S::ROWS, &bars[k]);
+            }
     }
-    const double2 *vt = g.v + ((long long)grp * 16) * S::NTB + tid;
-#if P8_VMODE == 3
-    // the middle stage's v' values are requested together with the tile: an L2 hit issued later queues behind the
-    // tile loads of the SM's other CTAs and costs a DRAM round trip (measured: 0.76 -> 0.83 of the HBM peak)
-    double2 vv[16];
-#pragma unroll
-    for (int m = 0; m < 16; ++m)
-        asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(vv[m].x), "=d"(vv[m].y) : "l"(vt + m * S::NTB));
-#endif
-    __syncthreads();
-    mbar_wait(bar, 0);
-#if P8_VMODE == 4
-    double2 vv[16];
-#pragma unroll
-    for (int m = 0; m < 16; ++m)
-        asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(vv[m].x), "=d"(vv[m].y) : "l"(vt + m * S::NTB));
-#endif
     // stage 1 / 3 task: (b0 = x0 mod 32, p); element (a0, q, r) at row q*N0 + a0*32 + b0, chunk (p*RQ + r) ^ (b0 & 7)
     const int b0 = tid % 32, p = tid / 32;
     cd tw[A0 - 1];
@@ -429,7 +429,16 @@ __global__ void __maxnreg__(P8_MAXREG_B) p8_mid(const __grid_constant__ CUtensor
     for (int k = 1; k < A0; ++k) tw[k - 1] = g.tw0[b0 * k];           // w_N0^(b0 k0a)
     // middle task: tid = ((k0a*NQ + q)*P + p)*RQ + r; element b0' at row q*N0 + k0a*32 + b0', chunk (p*RQ + r) ^ (b0' & 7)
     const int mr = tid % RQ, mp = (tid / RQ) % P, mq = (tid / (RQ * P)) % NQ, mk = tid / (RQ * P * NQ);
-    if (P8_SKEL_B != 2) {
+    const int rb = (mq * N0 + mk * 32) * 8, mc = mp * RQ + mr;
+    __syncthreads();                                    // mbarrier inits visible; from here on the groups are independent
+    if (pair >= g.n_pairs) return;
+    auto group_sync = [&]() {                           // named barrier 1 + gi over the group's 64 threads
+        if (gi == 0) asm volatile("bar.sync 1, %0;" ::"n"(S::NTB) : "memory");
+        else if (gi == 1) asm volatile("bar.sync 2, %0;" ::"n"(S::NTB) : "memory");
+        else asm volatile("bar.sync 3, %0;" ::"n"(S::NTB) : "memory");
+    };
+    static_assert(GB <= 3, "one named barrier per group");
+    mbar_wait(&bars[gi], 0);
     {
         cd u[A0 * B1];                                                  // u[a0*B1 + b1], b1 = q*RQ + r
 #pragma unroll
@@ -439,12 +448,12 @@ __global__ void __maxnreg__(P8_MAXREG_B) p8_mid(const __grid_constant__ CUtensor
 #pragma unroll
                 for (int r = 0; r < RQ; ++r)
                     u[a0 * B1 + q * RQ + r] = s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))];
-        if (P8_SKEL_B != 1 && P8_SKEL_B != 4) dft_rows<A0, B1, false>(u);
+        dft_rows<A0, B1, false>(u);
 #pragma unroll
         for (int k = 1; k < A0; ++k)
 #pragma unroll
             for (int c = 0; c < B1; ++c) u[k * B1 + c] = cmul(u[k * B1 + c], tw[k - 1]);
-        if (P8_SKEL_B != 1 && P8_SKEL_B != 4) dft_cols<A0, B1, false>(u);
+        dft_cols<A0, B1, false>(u);
 #pragma unroll
         for (int a0 = 0; a0 < A0; ++a0)
 #pragma unroll
@@ -453,36 +462,24 @@ __global__ void __maxnreg__(P8_MAXREG_B) p8_mid(const __grid_constant__ CUtensor
                 for (int r = 0; r < RQ; ++r)
                     s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))] = u[a0 * B1 + q * RQ + r];
     }
-    __syncthreads();
+    group_sync();
+    mbar_wait(&bars[GB], 0);                            // v' landed (requested before the tiles)
     {
         cd u[32];
-        const int rb = (mq * N0 + mk * 32) * 8, c = mp * RQ + mr;
 #pragma unroll
-        for (int b = 0; b < 32; ++b) u[b] = s[rb + b * 8 + (c ^ (b & 7))];
-#if P8_VMODE == 2
-        double2 vv[16];
+        for (int b = 0; b < 32; ++b) u[b] = s[rb + b * 8 + (mc ^ (b & 7))];
+        DFT<32, false>::run(u);
 #pragma unroll
         for (int m = 0; m < 16; ++m) {
-            if (P8_SKEL_B >= 3) vv[m] = make_double2(1.0 + tid, 2.0);
-            else asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(vv[m].x), "=d"(vv[m].y) : "l"(vt + m * S::NTB));
+            const double2 vv = vs[m * S::NTB + tid];
+            u[2 * m] = cscale(u[2 * m], vv.x);
+            u[2 * m + 1] = cscale(u[2 * m + 1], vv.y);
         }
-#endif
-        if (P8_SKEL_B != 1 && P8_SKEL_B != 4) DFT<32, false>::run(u);
-#if P8_VMODE == 0
-        double2 vv[16];
+        DFT<32, true>::run(u);
 #pragma unroll
-        for (int m = 0; m < 16; ++m) vv[m] = __ldg(vt + m * S::NTB);
-#endif
-#pragma unroll
-        for (int m = 0; m < 16; ++m) {
-            u[2 * m] = cscale(u[2 * m], vv[m].x);
-            u[2 * m + 1] = cscale(u[2 * m + 1], vv[m].y);
-        }
-        if (P8_SKEL_B != 1 && P8_SKEL_B != 4) DFT<32, true>::run(u);
-#pragma unroll
-        for (int b = 0; b < 32; ++b) s[rb + b * 8 + (c ^ (b & 7))] = u[b];
+        for (int b = 0; b < 32; ++b) s[rb + b * 8 + (mc ^ (b & 7))] = u[b];
     }
-    __syncthreads();
+    group_sync();
     {
         cd u[A0 * B1];
 #pragma unroll
@@ -492,12 +489,12 @@ __global__ void __maxnreg__(P8_MAXREG_B) p8_mid(const __grid_constant__ CUtensor
 #pragma unroll
                 for (int r = 0; r < RQ; ++r)
                     u[a0 * B1 + q * RQ + r] = s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))];
-        if (P8_SKEL_B != 1 && P8_SKEL_B != 4) dft_cols<A0, B1, true>(u);
+        dft_cols<A0, B1, true>(u);
 #pragma unroll
         for (int k = 1; k < A0; ++k)
 #pragma unroll
             for (int c = 0; c < B1; ++c) u[k * B1 + c] = cmulc(u[k * B1 + c], tw[k - 1]);
-        if (P8_SKEL_B != 1 && P8_SKEL_B != 4) dft_rows<A0, B1, true>(u);
+        dft_rows<A0, B1, true>(u);
 #pragma unroll
         for (int a0 = 0; a0 < A0; ++a0)
 #pragma unroll
@@ -506,11 +503,10 @@ __global__ void __maxnreg__(P8_MAXREG_B) p8_mid(const __grid_constant__ CUtensor
                 for (int r = 0; r < RQ; ++r)
                     s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))] = u[a0 * B1 + q * RQ + r];
     }
-    }
     fence_proxy_async();
-    __syncthreads();
+    group_sync();
     if (tid == 0) {
-        tensor_s2g_2d_sw(&map, grp * (P * RQ * 2), row0, s);
+        tensor_s2g_2d_sw(&map, grp_pos * (P * RQ * 2), pair * S::ROWS, s);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // shared memory must outlive the store's reads
     }

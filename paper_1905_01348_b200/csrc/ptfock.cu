@@ -163,7 +163,7 @@ struct P8Entry {
 template <class S> void launch_p8_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) { p8_fwd<S><<<grid, S::NT, S::SMEM_A, st>>>(a); }
 template <class S> void launch_p8_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) { p8_inv_acc<S><<<grid, S::NT, S::SMEM_C, st>>>(a); }
 template <class S> void launch_p8_mid(const CUtensorMap &m, const P8MidArgs &a, int pairs, cudaStream_t st) {
-    p8_mid<S><<<dim3(S::NGRP, pairs), S::NTB, S::SMEM_B, st>>>(m, a);
+    p8_mid<S><<<dim3(S::NGRP, (pairs + S::GB - 1) / S::GB), S::NTB * S::GB, S::SMEM_B, st>>>(m, a);
 }
 template <class S> cudaError_t prepare_p8() {
     cudaError_t e = cudaFuncSetAttribute(p8_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_A);
@@ -593,6 +593,7 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
         mark(w, 0);
         P8MidArgs b;
         b.v = p->v8_dev; b.tw0 = p->tw_dev[0];
+        b.n_pairs = ni * nj;
         p->p8->mid(p->tmap8, b, ni * nj, w.st);
         mark(w, 1);
         w.launches += 2;
