@@ -21,7 +21,16 @@
  * such a device ptfock_create returns PTFOCK_ERR_UNSUPPORTED_DEVICE (or PTFOCK_ERR_CUDA).
  *
  * Error behaviour: every function returns 0 (PTFOCK_OK) or a negative code below; nothing throws
- * or aborts across the ABI.  A plan is not thread-safe; distinct plans are independent.
+ * or aborts across the ABI.  A plan is not thread-safe (one host thread at a time); distinct plans are
+ * independent.  Calls on one plan may use different streams: the plan's scratch is shared by
+ * consecutive calls, so a call on another stream than the previous one first waits (on the device,
+ * cudaStreamWaitEvent) for the previous call to finish.  The caller's current device is left as it was.
+ *
+ * Supported grids: n0 in {16, 32, 48, 64, 120, 128}; (n1, n2) one of the built slab shapes
+ *   (64,64) (128,48) (48,48) (32,32) (90,60)            -- TMA-fed three-stage slab passes
+ *   (16,16) (16,32) (32,16) (16,48) (48,32) (32,64)     -- generic slab passes
+ * (all BASELINE.json configs, and the paper's own 60 x 90 x 120 grid stored as 120 x 90 x 60).
+ * 64 x 64 x 64 additionally has the two-stage slab passes + 32 x 32 pencil pass (the default there).
  */
 #ifndef PTFOCK_H
 #define PTFOCK_H
@@ -41,8 +50,9 @@ enum {
 
 enum {
     PTFOCK_OK = 0,
-    PTFOCK_ERR_INVALID_ARG = -1,        /* null pointer, negative count, n_targets > max_targets, bad enum ... */
-    PTFOCK_ERR_UNSUPPORTED_GRID = -2,   /* a grid edge outside {16, 32, 48, 64, 128} or a slab shape with no kernel */
+    PTFOCK_ERR_INVALID_ARG = -1,        /* null pointer, negative count, bad enum, pointer not on the plan's device,
+                                           n_targets > max_targets where a call says so ...                    */
+    PTFOCK_ERR_UNSUPPORTED_GRID = -2,   /* n0 or the slab shape (n1, n2) has no kernel (list above)             */
     PTFOCK_ERR_UNSUPPORTED_DEVICE = -3, /* device is not compute capability 10.x */
     PTFOCK_ERR_ALIGNMENT = -4,          /* an orbital pointer is not 16-byte aligned */
     PTFOCK_ERR_ALLOC = -5,              /* device or host allocation failed (workspace too small included) */
@@ -52,9 +62,11 @@ enum {
 
 typedef struct {
     double cell[9];           /* rows = lattice vectors a0, a1, a2 in bohr                                  */
-    int32_t n[3];             /* grid; each edge in {16, 32, 48, 64, 128}; index = (x0*n1 + x1)*n2 + x2     */
+    int32_t n[3];             /* grid (supported shapes: see above); index = (x0*n1 + x1)*n2 + x2           */
     int32_t n_occ;            /* number of Phi orbitals (N_i of Eq. 3's sum), >= 1                         */
-    int32_t max_targets;      /* largest n_targets one apply will be given (sizes the host-path staging)   */
+    int32_t max_targets;      /* largest n_targets of ptfock_apply_host and of ptfock_exchange_energy with
+                                 vx_psi == NULL (sizes their buffers) and the default wave; ptfock_apply
+                                 itself accepts any n_targets                                                */
     int32_t kernel;           /* PTFOCK_KERNEL_*                                                            */
     double omega;             /* bohr^-1; HSE only                                                          */
     double alpha;             /* mixing fraction multiplying V_X; 1.0 in all BASELINE configs */
@@ -114,11 +126,12 @@ int ptfock_last_cuda_error(void);
  *   info[0] = block_i, info[1] = block_j in use, info[2] = scratch bytes, info[3] = kernel launches
  *   issued by the most recent apply, info[4] = pair-solves executed by the most recent apply,
  *   info[5] = 1 if the most recent apply used the symmetric schedule, info[6] = total launches since create,
- *   info[7] = reserved. */
+ *   info[7] = 1 if the plan uses the two-stage slab passes + 32 x 32 pencil pass (pass8), else 0. */
 int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]);
 
 /* Test hook: W = IFFT[v' * FFT(conj(phi_i) psi_j)] for ONE pair through the same three kernels,
- * v' = -alpha/N * v (so V_X psi_j = sum_i phi_i W_ij).  w_out: one grid, device.  Asynchronous. */
+ * v' = -alpha/N * v (so V_X psi_j = sum_i phi_i W_ij).  w_out: one grid, device.  Asynchronous on `stream`
+ * (the first call allocates one grid of ones that the plan keeps). */
 int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const void *psi_j, void *w_out, void *stream);
 
 /* Per-pass device timing for the benchmark harness.  While on, every kernel launch of ptfock_apply is

@@ -24,7 +24,7 @@ EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_ap
            "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_copy_bandwidth"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "1886"]
 
 
 class PtfockError(RuntimeError):
@@ -206,7 +206,7 @@ class Plan:
         a = (ctypes.c_int64 * 8)()
         _check(lib().ptfock_plan_info(self._h, a), "ptfock_plan_info")
         return {"block_i": a[0], "block_j": a[1], "scratch_bytes": a[2], "last_launches": a[3], "last_pairs": a[4],
-                "last_symmetric": a[5], "total_launches": a[6]}
+                "last_symmetric": a[5], "total_launches": a[6], "pass8": a[7]}
 
     def set_profiling(self, on: bool):
         _check(lib().ptfock_set_profiling(self._h, 1 if on else 0), "ptfock_set_profiling")

@@ -212,26 +212,14 @@ __global__ void __launch_bounds__(kSlabThreads) slab_inv_acc(const SlabArgs g) {
     }
 }
 
-#ifndef PTF_PENCIL_MINB
-#define PTF_PENCIL_MINB 3
-#endif
-// ---- pass B ---------------------------------------------------------------------------------------
+// ---- pass B (n0 <= 48; longer pencils: pencil_tma.cuh, 64^3: pass8.cuh) ------------------------------------------
 // grid = (slab_pts / CW, pairs).  A CTA owns CW contiguous slab positions for all x0 of one pair.
 template <int N0> struct PencilShape {
-#ifndef PTF_PENCIL128_CW
-#define PTF_PENCIL128_CW 16
-#endif
-#ifndef PTF_PENCIL_CW
-#define PTF_PENCIL_CW 32
-#endif
-#ifndef PTF_PENCIL128_NT
-#define PTF_PENCIL128_NT (PTF_PENCIL128_CW * 8)
-#endif
-    static constexpr int CW = (N0 >= 120) ? PTF_PENCIL128_CW : PTF_PENCIL_CW;      // contiguous slab positions per CTA
+    static constexpr int CW = 32;                                  // contiguous slab positions per CTA
     static constexpr int R1 = Split<N0>::R1, R2 = Split<N0>::R2;
-    static constexpr int NT = (R2 == 1) ? 128 : (N0 >= 120 ? PTF_PENCIL128_NT : 256);
+    static constexpr int NT = (R2 == 1) ? 128 : 256;
     static constexpr int SMEM_BYTES = (R2 == 1) ? 0 : (N0 * CW + N0) * (int)sizeof(cd);
-    static constexpr int MINB = (N0 >= 120) ? 512 / NT : (R2 == 1 ? 1 : PTF_PENCIL_MINB);   // 128: two CTAs (128 regs) share an SM
+    static constexpr int MINB = (R2 == 1) ? 1 : 3;
 };
 
 struct PencilArgs {

@@ -3,7 +3,6 @@
 // PAPER.md:149 "Batched implementation"; i <= j pair symmetry when Psi = Phi).
 #include "../../include/ptfock.h"
 #include "kernels.cuh"
-#include "slab2.cuh"
 #include "slabx.cuh"
 #include "pencil_tma.cuh"
 #include "pass8.cuh"
@@ -30,6 +29,19 @@ thread_local int g_last_cuda = 0;
         }                                                     \
     } while (0)
 
+// makes `device` current for the duration of a call and restores the caller's device afterwards
+struct DeviceGuard {
+    int prev;
+    cudaError_t err;
+    explicit DeviceGuard(int device) : prev(-1), err(cudaSuccess) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+        else if (err == cudaSuccess) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define GUARD(dev) DeviceGuard guard__(dev); CU(guard__.err)
+
 typedef void (*slab_launch_fn)(const SlabArgs &, dim3, cudaStream_t);
 typedef void (*pencil_launch_fn)(const PencilArgs &, int pairs, cudaStream_t);
 
@@ -52,7 +64,6 @@ struct SlabEntry {
     int ax1_r1, ax1_r2, ax2_r1, ax2_r2;     // digit split per axis: position k1*r2 + k2 holds frequency k1 + r1*k2
     int nt3;                                // 0: scratch slab is [pos1][pos2]; else slabx's free layout
                                             //    s = m*nt3 + k2a*n1 + k1  (k1 natural), k2 = k2a + ax2_r1*m
-    int legacy;                             // 1: pre-slabx kernel (selected by PTFOCK_SLAB=legacy, for comparisons)
 };
 
 template <int N1, int N2> cudaError_t prepare_slab() {
@@ -63,18 +74,6 @@ template <int N1, int N2> cudaError_t prepare_slab() {
                                 SlabShape<N1, N2>::SMEM_BYTES);
 }
 
-// register-resident 3-stage kernels (slab2.cuh)
-template <class S> void launch_slab2_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
-    slab2_fwd<S><<<grid, S::NT, S::SMEM_BYTES, st>>>(a);
-}
-template <class S> void launch_slab2_inv(const SlabArgs &a, dim3 grid, cudaStream_t st) {
-    slab2_inv_acc<S><<<grid, S::NT, S::SMEM_BYTES, st>>>(a);
-}
-template <class S> cudaError_t prepare_slab2() {
-    cudaError_t e = cudaFuncSetAttribute(slab2_fwd<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(slab2_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES);
-}
 // TMA-fed in-place kernels (slabx.cuh)
 template <class S> void launch_slabx_fwd(const SlabArgs &a, dim3 grid, cudaStream_t st) {
     slabx_fwd<S><<<grid, S::NT, S::SMEM_A, st>>>(a);
@@ -87,41 +86,22 @@ template <class S> cudaError_t prepare_slabx() {
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(slabx_inv_acc<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_C);
 }
-//          N1   N2  A1  B1  A2  B2  kind Q  bulk stores
-#ifndef PTF_TS64
-#define PTF_TS64 true
-#endif
-typedef SX<64, 64, 16, 4, 4, 16, false, PTF_TS64> SX_64x64;
-#ifndef PTF_P128
+//          N1   N2  A1  B1  A2  B2  kind Q  bulk stores  CTAs/SM
+typedef SX<64, 64, 16, 4, 4, 16, false, true> SX_64x64;
 typedef SX<128, 48, 8, 16, 3, 16, true, false> SX_128x48;     // kind Q: 256 threads, 24-point first stage
-#else
-typedef SX<128, 48, 16, 8, 3, 16, false, false> SX_128x48;    // kind P: 384 threads, 24-point middle stage (spills: slower)
-#endif
-#ifndef PTF_SMALL_MINB
-#define PTF_SMALL_MINB 2      // 36 KB / 16 KB tiles: two CTAs per SM (128 registers) run out of phase
-#endif
-typedef SX<48, 48, 3, 16, 3, 16, true, false, PTF_SMALL_MINB> SX_48x48;        // kind Q: 9-point first stage, 144-task DFT16 stages
-typedef SX<32, 32, 2, 16, 2, 16, true, false, PTF_SMALL_MINB> SX_32x32;
+typedef SX<48, 48, 3, 16, 3, 16, true, false, 2> SX_48x48;    // kind Q: 9-point first stage, 144-task DFT16 stages; 36 KB tiles, 128 registers
+typedef SX<32, 32, 2, 16, 2, 16, true, false, 2> SX_32x32;
 typedef SX<90, 60, 6, 15, 4, 15, true, false> SX_90x60;        // paper grid 120 x 90 x 60: 24-point first stage, DFT15 stages
-#define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3, 0 }
-//            N1   N2  A1  B1  A2  B2  min CTAs/SM
-typedef Slab2<64, 64, 4, 16, 16, 4, 1> S2_64x64;
-typedef Slab2<128, 48, 8, 16, 16, 3, 1> S2_128x48;
-typedef Slab2<48, 48, 3, 16, 16, 3, 3> S2_48x48;
-typedef Slab2<32, 32, 2, 16, 16, 2, 8> S2_32x32;
-
-#define SLAB2(S) { S::N1, S::N2, launch_slab2_fwd<S>, launch_slab2_inv<S>, prepare_slab2<S>, S::A1, S::B1, S::A2, S::B2, 0, 1 }
+#define SLABX(S) { S::N1, S::N2, launch_slabx_fwd<S>, launch_slabx_inv<S>, prepare_slabx<S>, S::A1, S::B1, S::A2, S::B2, S::TS ? 0 : S::NT3 }
 #define SLAB(N1, N2) { N1, N2, launch_slab_fwd<N1, N2>, launch_slab_inv<N1, N2>, prepare_slab<N1, N2>, \
-                       Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2, 0, 1 }
-// first match wins: the 3-stage kernels serve the BASELINE shapes, the generic 4-stage ones the rest
+                       Split<N1>::R1, Split<N1>::R2, Split<N2>::R1, Split<N2>::R2, 0 }
+// the TMA-fed 3-stage kernels serve the BASELINE slab shapes, the generic 4-stage ones the small / mixed ones
 const SlabEntry kSlabs[] = {
     SLABX(SX_64x64), SLABX(SX_128x48), SLABX(SX_48x48), SLABX(SX_32x32), SLABX(SX_90x60),
-    SLAB2(S2_64x64), SLAB2(S2_128x48), SLAB2(S2_48x48), SLAB2(S2_32x32),
-    SLAB(16, 16), SLAB(32, 32), SLAB(48, 48), SLAB(64, 64), SLAB(128, 48),
-    SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),
+    SLAB(16, 16), SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),
 };
 #undef SLAB
-#undef SLAB2
+#undef SLABX
 
 typedef void (*pencil_tma_launch_fn)(const CUtensorMap &, const PencilTmaArgs &, int pairs, cudaStream_t);
 struct PencilEntry {
@@ -144,7 +124,7 @@ template <int N0> cudaError_t prepare_pencil() {
     return cudaFuncSetAttribute(pencil_mid<N0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 PencilShape<N0>::SMEM_BYTES);
 }
-#define PENCIL(N0) { N0, launch_pencil<N0>, prepare_pencil<N0>, launch_pencil_tma<N0>, prepare_pencil_tma<N0>, PencilTma<N0>::CW }
+#define PENCIL(N0) { N0, nullptr, nullptr, launch_pencil_tma<N0>, prepare_pencil_tma<N0>, PencilTma<N0>::CW }
 #define PENCIL_REG(N0) { N0, launch_pencil<N0>, prepare_pencil<N0>, nullptr, nullptr, 0 }
 // the tensor-map variant serves the long pencils; at n0 <= 48 its 16-wide tiles leave most threads idle (measured slower)
 const PencilEntry kPencils[] = { PENCIL_REG(16), PENCIL_REG(32), PENCIL_REG(48), PENCIL(64), PENCIL(128), PENCIL(120) };
@@ -228,6 +208,13 @@ struct ptfock_plan {
     cd *st_phi, *st_psi, *st_out;
     cudaStream_t copy_stream;           // host path: copies run here, chunk by chunk, overlapped with the waves
     std::vector<cudaEvent_t> *copy_ev;
+    int sm_count;
+    cd *ones;                           // ptfock_debug_pair: a grid of ones (lazily allocated)
+    // cross-stream ordering: the plan's scratch is shared by consecutive calls, so a call on another stream first
+    // waits for the event the previous call recorded at its end
+    cudaEvent_t busy_ev;
+    cudaStream_t last_stream;
+    int has_last;
     // statistics
     long long last_launches, last_pairs, total_launches;
     int last_symmetric;
@@ -268,6 +255,8 @@ void free_plan(ptfock_plan *p) {
     cudaFree(p->st_phi);
     cudaFree(p->st_psi);
     cudaFree(p->st_out);
+    cudaFree(p->ones);
+    if (p->busy_ev) cudaEventDestroy(p->busy_ev);
     if (p->ev_pool) { for (cudaEvent_t e : *p->ev_pool) cudaEventDestroy(e); delete p->ev_pool; }
     if (p->copy_ev) { for (cudaEvent_t e : *p->copy_ev) cudaEventDestroy(e); delete p->copy_ev; }
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
@@ -374,10 +363,8 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (!std::isfinite(d.alpha)) return PTFOCK_ERR_INVALID_ARG;
     for (int k = 0; k < 3; ++k) if (!edge_ok(d.n[k])) return PTFOCK_ERR_UNSUPPORTED_GRID;
     const SlabEntry *slab = nullptr;
-    const char *pick = std::getenv("PTFOCK_SLAB");          // "legacy": the pre-slabx kernels (comparison runs only)
-    const bool legacy_only = pick && std::strcmp(pick, "legacy") == 0;
     for (const SlabEntry &e : kSlabs)
-        if (!slab && e.n1 == d.n[1] && e.n2 == d.n[2] && (!legacy_only || e.legacy)) slab = &e;
+        if (!slab && e.n1 == d.n[1] && e.n2 == d.n[2]) slab = &e;
     const PencilEntry *pencil = nullptr;
     for (const PencilEntry &e : kPencils) if (e.n0 == d.n[0]) pencil = &e;
     if (!slab || !pencil) return PTFOCK_ERR_UNSUPPORTED_GRID;
@@ -392,7 +379,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     cudaDeviceProp prop;
     CU(cudaGetDeviceProperties(&prop, d.device));
     if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;     // sm_100a code only, no fallback
-    CU(cudaSetDevice(d.device));
+    GUARD(d.device);
 
     ptfock_plan *p = new (std::nothrow) ptfock_plan();
     if (!p) return PTFOCK_ERR_ALLOC;
@@ -404,6 +391,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     p->slab = slab;
     p->pencil = pencil;
     p->p8 = p8;
+    p->sm_count = prop.multiProcessorCount;
 
     std::vector<double> vperm;
     bool even = false;
@@ -420,7 +408,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
         CUP(cudaMemcpy(p->v8_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
     } else {
         CUP(slab->prepare());
-        CUP(pencil->prepare());
+        if (pencil->prepare) CUP(pencil->prepare());
         CUP(cudaMalloc(&p->v_dev, sizeof(double) * p->N));
         CUP(cudaMemcpy(p->v_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
     }
@@ -458,16 +446,33 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (Ib > d.n_occ) Ib = d.n_occ;
     if (Jb > d.max_targets) Jb = d.max_targets;
     const size_t pair_bytes = sizeof(cd) * (size_t)p->N;
-    const size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)12 << 30);
+    // default scratch: at most 12 GiB and at most 60 % of what is free now (Phi of Si1536 alone is 39 GB)
+    size_t limit = d.workspace_bytes ? (size_t)d.workspace_bytes : ((size_t)12 << 30);
+    if (!d.workspace_bytes) {
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b / 10 * 6 < limit) limit = free_b / 10 * 6;
+        if (limit < pair_bytes) limit = pair_bytes;
+    }
     while ((long long)Ib * Jb > 65535 && Ib > 1) Ib = (Ib + 1) / 2;     // pass B puts the wave's pairs on gridDim.y
     while ((long long)Ib * Jb > 65535 && Jb > 1) Jb = (Jb + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Jb > 1) Jb = (Jb + 1) / 2;
     if ((size_t)Ib * Jb * pair_bytes > limit) { free_plan(p); return PTFOCK_ERR_ALLOC; }
+    // a failing allocation (fragmentation, another allocator holding the memory) shrinks the wave instead of failing
+    for (;;) {
+        p->scratch_bytes = (size_t)Ib * Jb * pair_bytes;
+        cudaError_t e = cudaMalloc(&p->scratch, p->scratch_bytes);
+        if (e == cudaSuccess) break;
+        cudaGetLastError();
+        p->scratch = nullptr;
+        if (e != cudaErrorMemoryAllocation || d.workspace_bytes || (Ib == 1 && Jb == 1)) {
+            g_last_cuda = (int)e; free_plan(p); return PTFOCK_ERR_ALLOC;
+        }
+        if (Ib > 1) Ib = (Ib + 1) / 2; else Jb = (Jb + 1) / 2;
+    }
     p->Ib = Ib;
     p->Jb = Jb;
-    p->scratch_bytes = (size_t)Ib * Jb * pair_bytes;
-    CUP(cudaMalloc(&p->scratch, p->scratch_bytes));
+    CUP(cudaEventCreateWithFlags(&p->busy_ev, cudaEventDisableTiming));
     p->use_tma = 0;
     {
         typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -488,17 +493,17 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) { g_last_cuda = (int)r; free_plan(p); return PTFOCK_ERR_CUDA; }
-        } else if (pencil->run_tma && have) {
+        } else if (pencil->run_tma) {
+            if (!have) { free_plan(p); return PTFOCK_ERR_CUDA; }
             const cuuint64_t dims[2] = { (cuuint64_t)2 * p->slab_pts, (cuuint64_t)Ib * Jb * d.n[0] };
             const cuuint64_t strides[1] = { (cuuint64_t)p->slab_pts * sizeof(cd) };
             const cuuint32_t box[2] = { (cuuint32_t)(2 * pencil->tma_cw), (cuuint32_t)d.n[0] };
             CUresult r = ((encode_fn)fn)(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            if (r == CUDA_SUCCESS) {
-                CUP(pencil->prepare_tma());
-                p->use_tma = 1;
-            }
+            if (r != CUDA_SUCCESS) { g_last_cuda = (int)r; free_plan(p); return PTFOCK_ERR_CUDA; }
+            CUP(pencil->prepare_tma());
+            p->use_tma = 1;
         }
     }
     CUP(cudaMalloc(&p->partials, sizeof(double2) * 1024));
@@ -511,7 +516,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
 
 extern "C" int ptfock_destroy(ptfock_plan *plan) {
     if (!plan) return PTFOCK_OK;
-    cudaSetDevice(plan->d.device);
+    DeviceGuard guard(plan->d.device);
     cudaDeviceSynchronize();
     free_plan(plan);
     return PTFOCK_OK;
@@ -521,7 +526,7 @@ extern "C" const char *ptfock_strerror(int code) {
     switch (code) {
         case PTFOCK_OK: return "ok";
         case PTFOCK_ERR_INVALID_ARG: return "invalid argument";
-        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (edges must be in {16,32,48,64,128} with a built slab shape)";
+        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (n0 in {16,32,48,64,120,128}; (n1,n2) one of the built slab shapes, see ptfock.h)";
         case PTFOCK_ERR_UNSUPPORTED_DEVICE: return "unsupported device (needs compute capability 10.x; there is no CPU fallback)";
         case PTFOCK_ERR_ALIGNMENT: return "pointer not 16-byte aligned";
         case PTFOCK_ERR_ALLOC: return "allocation failed or workspace too small";
@@ -542,7 +547,7 @@ extern "C" int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]) {
     info[4] = plan->last_pairs;
     info[5] = plan->last_symmetric;
     info[6] = plan->total_launches;
-    info[7] = 0;
+    info[7] = plan->p8 ? 1 : 0;
     return PTFOCK_OK;
 }
 
@@ -555,7 +560,22 @@ struct Wave {
     ptfock_plan *p;
     cudaStream_t st;
     long long launches, pairs;
+    cudaError_t err;                    // first failure of an event / wait / launch in this call
+    void note(cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; }
 };
+
+// every call that touches the plan's buffers starts with begin_call and ends with end_call: a call on another stream
+// than the previous one waits for the previous call's end (the scratch, the energy buffer and the staging buffers
+// are shared by consecutive calls)
+cudaError_t begin_call(ptfock_plan *p, cudaStream_t st) {
+    if (p->has_last && p->last_stream != st) return cudaStreamWaitEvent(st, p->busy_ev, 0);
+    return cudaSuccess;
+}
+cudaError_t end_call(ptfock_plan *p, cudaStream_t st) {
+    cudaError_t e = cudaEventRecord(p->busy_ev, st);
+    if (e == cudaSuccess) { p->last_stream = st; p->has_last = 1; }
+    return e;
+}
 
 // profiling: record an event that closes an interval of kind `tag` (-1: opens a new run of intervals)
 void mark(Wave &w, int tag) {
@@ -564,11 +584,12 @@ void mark(Wave &w, int tag) {
     if (!p->ev_pool) { p->ev_pool = new std::vector<cudaEvent_t>(); p->ev_tags = new std::vector<int>(); }
     if (p->ev_used == p->ev_pool->size()) {
         cudaEvent_t e;
-        if (cudaEventCreate(&e) != cudaSuccess) return;
+        const cudaError_t ce = cudaEventCreate(&e);
+        if (ce != cudaSuccess) { w.note(ce); return; }
         p->ev_pool->push_back(e);
         p->ev_tags->push_back(-1);
     }
-    cudaEventRecord((*p->ev_pool)[p->ev_used], w.st);
+    w.note(cudaEventRecord((*p->ev_pool)[p->ev_used], w.st));
     (*p->ev_tags)[p->ev_used] = tag;
     p->ev_used++;
 }
@@ -585,7 +606,7 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
     // split the i loop over blockIdx.z until the grid has a few CTAs per SM
     int z = 1;
     const long long base = (long long)p->d.n[0] * nj;
-    while (z < ni && base * z * (p->p8 ? p->p8->nq : 1) < 148LL * (p->p8 ? 12 : 6)) z *= 2;
+    while (z < ni && base * z * (p->p8 ? p->p8->nq : 1) < (long long)p->sm_count * (p->p8 ? 12 : 6)) z *= 2;
     if (z > ni) z = ni;
     mark(w, -1);
     if (p->p8) {
@@ -630,6 +651,7 @@ void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, in
     else p->slab->inv(a, dim3(nt, p->d.n[0], 1), w.st);
     mark(w, 2);
     w.launches += 1;
+    w.note(cudaPeekAtLastError());
 }
 
 bool overlaps(const void *a, size_t na, const void *b, size_t nb) {
@@ -643,6 +665,15 @@ int check_apply_args(const ptfock_plan *p, const void *phi, const void *psi, int
     if (!out && n_targets > 0) return PTFOCK_ERR_INVALID_ARG;
     if (!psi && (self_offset < 0 || (long long)self_offset + n_targets > p->d.n_occ)) return PTFOCK_ERR_INVALID_ARG;
     if (((uintptr_t)phi | (uintptr_t)psi | (uintptr_t)out) & 15) return PTFOCK_ERR_ALIGNMENT;
+    // device pointers on the plan's device (managed memory is accepted)
+    const void *ptrs[3] = { phi, psi, out };
+    for (const void *q : ptrs) {
+        if (!q) continue;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, q) != cudaSuccess) { cudaGetLastError(); return PTFOCK_ERR_INVALID_ARG; }
+        if (at.type == cudaMemoryTypeManaged) continue;
+        if (at.type != cudaMemoryTypeDevice || at.device != p->d.device) return PTFOCK_ERR_INVALID_ARG;
+    }
     return PTFOCK_OK;
 }
 
@@ -653,9 +684,14 @@ struct HostPipe {
     std::vector<cudaEvent_t> *ev;       // [0, n_chunks): Phi chunk landed; [n_chunks]: Psi landed; [n_chunks + 1]: scratch event
     int chunk, n_chunks;
     std::vector<char> waited;
+    cudaError_t err = cudaSuccess;
     void need(cudaStream_t st, int lo, int hi) {                  // orbitals [lo, hi) of Phi
         for (int c = lo / chunk; c <= (hi - 1) / chunk && c < n_chunks; ++c)
-            if (!waited[c]) { cudaStreamWaitEvent(st, (*ev)[c], 0); waited[c] = 1; }
+            if (!waited[c]) {
+                const cudaError_t e = cudaStreamWaitEvent(st, (*ev)[c], 0);
+                if (e != cudaSuccess && err == cudaSuccess) err = e;
+                waited[c] = 1;
+            }
     }
 };
 
@@ -665,9 +701,8 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
     if (n_targets == 0) { p->last_launches = 0; p->last_pairs = 0; p->last_symmetric = 0; return PTFOCK_OK; }
     if (overlaps(out, gbytes * n_targets, phi, gbytes * p->d.n_occ)) return PTFOCK_ERR_ALIAS;
     if (psi && overlaps(out, gbytes * n_targets, psi, gbytes * n_targets)) return PTFOCK_ERR_ALIAS;
-    CU(cudaSetDevice(p->d.device));
     CU(cudaMemsetAsync(out, 0, gbytes * n_targets, st));             // Alg. 2 line 1
-    Wave w{ p, st, 0, 0 };
+    Wave w{ p, st, 0, 0, cudaSuccess };
     const int n_occ = p->d.n_occ;
     const bool symmetric = (!psi) && self_offset == 0 && n_targets == n_occ && p->v_even && n_occ > 1;
     if (symmetric) {
@@ -690,7 +725,7 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
         if (hp) {
             // host path: i blocks outermost, so every chunk of Phi is used by all j-blocks as soon as it has landed
             // and the rest of the copy hides behind those waves (out_j accumulates over the waves in any order)
-            if (psi) cudaStreamWaitEvent(st, (*hp->ev)[hp->n_chunks], 0);
+            if (psi) w.note(cudaStreamWaitEvent(st, (*hp->ev)[hp->n_chunks], 0));
             else hp->need(st, self_offset, self_offset + n_targets);
             for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
                 const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
@@ -712,7 +747,9 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
             }
         }
     }
-    CU(cudaGetLastError());
+    if (hp) w.note(hp->err);
+    w.note(cudaGetLastError());
+    if (w.err != cudaSuccess) { g_last_cuda = (int)w.err; return PTFOCK_ERR_CUDA; }
     p->last_launches = w.launches;
     p->last_pairs = w.pairs;
     p->last_symmetric = symmetric ? 1 : 0;
@@ -726,7 +763,12 @@ extern "C" int ptfock_apply(ptfock_plan *plan, const void *phi, const void *psi,
                             int32_t n_targets, void *out, void *stream) {
     int rc = check_apply_args(plan, phi, psi, self_offset, n_targets, out);
     if (rc != PTFOCK_OK) return rc;
-    return apply_device(plan, (const cd *)phi, (const cd *)psi, self_offset, n_targets, (cd *)out, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    rc = apply_device(plan, (const cd *)phi, (const cd *)psi, self_offset, n_targets, (cd *)out, st);
+    CU(end_call(plan, st));
+    return rc;
 }
 
 extern "C" int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const void *psi, int32_t self_offset,
@@ -735,8 +777,9 @@ extern "C" int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const 
     if (!psi && (self_offset < 0 || (long long)self_offset + n_targets > plan->d.n_occ)) return PTFOCK_ERR_INVALID_ARG;
     if (((uintptr_t)phi | (uintptr_t)psi | (uintptr_t)vx_psi) & 15) return PTFOCK_ERR_ALIGNMENT;
     cudaStream_t st = (cudaStream_t)stream;
-    CU(cudaSetDevice(plan->d.device));
+    GUARD(plan->d.device);
     if (n_targets == 0) { *e_host = 0.0; return PTFOCK_OK; }
+    CU(begin_call(plan, st));
     const cd *vx = (const cd *)vx_psi;
     if (!vx) {
         if (n_targets > plan->d.max_targets) return PTFOCK_ERR_INVALID_ARG;
@@ -757,6 +800,7 @@ extern "C" int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const 
     plan->total_launches += 2;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(plan->result_host, plan->result_dev, sizeof(double2), cudaMemcpyDeviceToHost, st));
+    CU(end_call(plan, st));
     CU(cudaStreamSynchronize(st));
     *e_host = plan->result_host->x;
     return PTFOCK_OK;
@@ -767,7 +811,7 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     if (!plan || !phi_host || !out_host || n_targets < 0 || n_targets > plan->d.max_targets) return PTFOCK_ERR_INVALID_ARG;
     if (!psi_host && (self_offset < 0 || (long long)self_offset + n_targets > plan->d.n_occ)) return PTFOCK_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    CU(cudaSetDevice(plan->d.device));
+    GUARD(plan->d.device);
     const size_t gbytes = sizeof(cd) * (size_t)plan->N;
     auto ensure = [&](cd **buf, size_t bytes) -> int {
         if (*buf) return PTFOCK_OK;
@@ -793,12 +837,16 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     }
     hp.ev = plan->copy_ev;
     hp.waited.assign(hp.n_chunks, 0);
+    CU(begin_call(plan, st));
     // the copy stream starts after whatever the caller queued on `stream` (the event slot [n_chunks + 1] is free here)
     CU(cudaEventRecord((*hp.ev)[hp.n_chunks + 1], st));
     CU(cudaStreamWaitEvent(hp.cs, (*hp.ev)[hp.n_chunks + 1], 0));
+    // from here on async copies out of the caller's host buffers may be in flight: every exit drains the copy stream
+#define CUH(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_cuda = (int)e__; cudaStreamSynchronize(hp.cs); \
+        cudaStreamSynchronize(st); return PTFOCK_ERR_CUDA; } } while (0)
     if (psi_host) {
-        CU(cudaMemcpyAsync(plan->st_psi, psi_host, gbytes * n_targets, cudaMemcpyHostToDevice, hp.cs));
-        CU(cudaEventRecord((*hp.ev)[hp.n_chunks], hp.cs));
+        CUH(cudaMemcpyAsync(plan->st_psi, psi_host, gbytes * n_targets, cudaMemcpyHostToDevice, hp.cs));
+        CUH(cudaEventRecord((*hp.ev)[hp.n_chunks], hp.cs));
     }
     // chunks that hold the targets (Psi = Phi[self_offset...]) go first, the rest in the order the i loop reads them
     std::vector<int> order;
@@ -807,42 +855,46 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     for (int c = 0; c < hp.n_chunks; ++c) if (c < t_lo || c > t_hi) order.push_back(c);
     for (int c : order) {
         const int lo = c * hp.chunk, cnt = (plan->d.n_occ - lo < hp.chunk) ? plan->d.n_occ - lo : hp.chunk;
-        CU(cudaMemcpyAsync(plan->st_phi + (size_t)lo * plan->N, (const cd *)phi_host + (size_t)lo * plan->N, gbytes * cnt,
+        CUH(cudaMemcpyAsync(plan->st_phi + (size_t)lo * plan->N, (const cd *)phi_host + (size_t)lo * plan->N, gbytes * cnt,
                            cudaMemcpyHostToDevice, hp.cs));
-        CU(cudaEventRecord((*hp.ev)[c], hp.cs));
+        CUH(cudaEventRecord((*hp.ev)[c], hp.cs));
     }
     rc = apply_device(plan, plan->st_phi, psi_host ? plan->st_psi : nullptr, self_offset, n_targets, plan->st_out, st, &hp);
-    if (rc != PTFOCK_OK) { cudaStreamSynchronize(hp.cs); return rc; }
-    CU(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
-    CU(cudaStreamSynchronize(hp.cs));
+    if (rc != PTFOCK_OK) { cudaStreamSynchronize(hp.cs); cudaStreamSynchronize(st); return rc; }
+    CUH(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
+    CUH(end_call(plan, st));
+    CUH(cudaStreamSynchronize(st));
+    CUH(cudaStreamSynchronize(hp.cs));
     return PTFOCK_OK;
+#undef CUH
 }
 
 extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const void *psi_j, void *w_out, void *stream) {
     if (!plan || !phi_i || !psi_j || !w_out) return PTFOCK_ERR_INVALID_ARG;
     if (((uintptr_t)phi_i | (uintptr_t)psi_j | (uintptr_t)w_out) & 15) return PTFOCK_ERR_ALIGNMENT;
     cudaStream_t st = (cudaStream_t)stream;
-    CU(cudaSetDevice(plan->d.device));
+    GUARD(plan->d.device);
     const size_t gbytes = sizeof(cd) * (size_t)plan->N;
-    cd *ones = nullptr;
-    cudaError_t e = cudaMalloc(&ones, gbytes);
-    if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
-    fill_ones<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(ones, plan->N);
-    cudaMemsetAsync(w_out, 0, gbytes, st);
-    Wave w{ plan, st, 0, 0 };
+    CU(begin_call(plan, st));
+    if (!plan->ones) {
+        cudaError_t e = cudaMalloc(&plan->ones, gbytes);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
+        fill_ones<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(plan->ones, plan->N);
+    }
+    CU(cudaMemsetAsync(w_out, 0, gbytes, st));
+    Wave w{ plan, st, 0, 0, cudaSuccess };
     wave_forward_mid(w, (const cd *)phi_i, (const cd *)psi_j, 0, 1, 0, 1);
-    wave_accumulate(w, ones, 0, 1, (cd *)w_out, 0, 1, 1, 1, 0);
+    wave_accumulate(w, plan->ones, 0, 1, (cd *)w_out, 0, 1, 1, 1, 0);
     plan->total_launches += w.launches + 1;
-    cudaError_t e2 = cudaStreamSynchronize(st);
-    cudaFree(ones);
-    if (e2 != cudaSuccess) { g_last_cuda = (int)e2; return PTFOCK_ERR_CUDA; }
+    w.note(cudaGetLastError());
+    if (w.err != cudaSuccess) { g_last_cuda = (int)w.err; return PTFOCK_ERR_CUDA; }
+    CU(end_call(plan, st));
     return PTFOCK_OK;
 }
 
 extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
     if (!tflops_host) return PTFOCK_ERR_INVALID_ARG;
-    CU(cudaSetDevice(device));
+    GUARD(device);
     cudaDeviceProp prop;
     CU(cudaGetDeviceProperties(&prop, device));
     if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
@@ -873,7 +925,7 @@ extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
 
 extern "C" int ptfock_measure_copy_bandwidth(int32_t device, uint64_t bytes, int32_t reps, double *gbs_host) {
     if (!gbs_host || bytes < 4096 || reps < 1) return PTFOCK_ERR_INVALID_ARG;
-    CU(cudaSetDevice(device));
+    GUARD(device);
     cudaDeviceProp prop;
     CU(cudaGetDeviceProperties(&prop, device));
     if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
@@ -917,7 +969,7 @@ extern "C" int ptfock_get_profile(ptfock_plan *plan, double ms[3], int64_t launc
     if (!plan || !ms || !launches) return PTFOCK_ERR_INVALID_ARG;
     for (int k = 0; k < 3; ++k) { ms[k] = 0.0; launches[k] = 0; }
     if (plan->ev_pool && plan->ev_used > 0) {
-        CU(cudaSetDevice(plan->d.device));
+        GUARD(plan->d.device);
         CU(cudaEventSynchronize((*plan->ev_pool)[plan->ev_used - 1]));
         for (size_t k = 1; k < plan->ev_used; ++k) {
             const int tag = (*plan->ev_tags)[k];

@@ -62,8 +62,21 @@ def test_Si512_nonself_full(cuda_device):
         info = plan.info()
         e = plan.exchange_energy(phi, psi, vx_psi=out)
     assert info["last_symmetric"] == 0 and info["last_pairs"] == 1024 * 1024
-    _check_cols(cfg, phi, psi, out, [0, 511, 1023])
-    assert np.isfinite(e)
+    # first / last columns of j-tiles and tile interiors (J_b = 16): 0, 5 | 517 | 1000, 1023
+    cols = [0, 5, 517, 1000, 1023]
+    ref = _oracle_columns(cfg, phi.cpu().numpy(), np.ascontiguousarray(psi[cols].cpu().numpy()))
+    got = out[cols].cpu().numpy()
+    assert float(np.abs(got - ref).max() / np.abs(ref).max()) <= TOL
+    # E_x = sum over ALL columns of the library's result, so the check is: the library's dot-product reduction agrees with
+    # the oracle's formula applied to the library's own V_X Psi (pins the reduction and the 1/2 Omega/N prefactor at full
+    # size), and the sampled columns' contributions agree with the oracle's columns
+    e_lib_cols = oracle.exchange_energy(cfg.cell, cfg.n, psi[cols].cpu().numpy(), got).real
+    e_ref_cols = oracle.exchange_energy(cfg.cell, cfg.n, psi[cols].cpu().numpy(), ref).real
+    assert abs(e_lib_cols - e_ref_cols) <= TOL * abs(e_ref_cols)
+    with binding.plan_for(cfg, max_targets=len(cols)) as plan2:
+        e_cols = plan2.exchange_energy(phi, psi[cols].contiguous())
+    assert abs(e_cols - e_ref_cols) <= TOL * abs(e_ref_cols) and e_cols < 0.0
+    assert np.isfinite(e) and e < e_cols
 
 
 def test_Si1536_streamed_j_blocks(cuda_device):
@@ -73,13 +86,14 @@ def test_Si1536_streamed_j_blocks(cuda_device):
     host = phi.cpu().numpy()
     with binding.plan_for(cfg) as plan:
         out = torch.empty((cfg.j_block,) + cfg.n, dtype=torch.complex128, device=cuda_device)
-        for offset, col in ((0, 0), (1536, 95)):
+        # one tile-edge and one tile-interior column (J_b = 8) per block
+        for offset, cols in ((0, [0, 43]), (1536, [50, 95])):
             plan.apply(phi, None, out=out, self_offset=offset, n_targets=cfg.j_block)
             torch.cuda.synchronize()
             assert plan.info()["last_pairs"] == 96 * 3072
-            ref = _oracle_columns(cfg, host, host[offset + col:offset + col + 1])
-            got = out[col].cpu().numpy()
-            err = float(np.abs(got - ref[0]).max() / np.abs(ref[0]).max())
+            ref = _oracle_columns(cfg, host, np.ascontiguousarray(host[[offset + c for c in cols]]))
+            got = out[cols].cpu().numpy()
+            err = float(np.abs(got - ref).max() / np.abs(ref).max())
             assert err <= TOL, (offset, err)
 
 

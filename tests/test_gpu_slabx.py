@@ -113,26 +113,3 @@ def test_repeated_applies_are_bit_identical(cuda_device, shape):
             assert torch.equal(first, again)
     ref = _oracle(cfg, phi, psi[[0, 8]].contiguous())
     assert _rel(first[[0, 8]].cpu().numpy(), ref) <= TOL
-
-
-@pytest.mark.parametrize("shape", [SHAPES[0], SHAPES[1]], ids=[SHAPES[0][0], SHAPES[1][0]])
-def test_comparison_paths_match_oracle(cuda_device, shape, monkeypatch):
-    """PTFOCK_SLAB=legacy / PTFOCK_PENCIL=legacy select the pre-TMA kernels for A/B comparisons in bench runs (read at
-    ptfock_create); they must stay correct too.  x0 = 64 here so that the default plan uses the tensor-map pencil."""
-    name, edges, _ = shape
-    n = (64,) + tuple(shape[2][1:])
-    cfg = synth.Config(name + "_cmp", (41.04,) + tuple(edges[1:]), n, 3, synth.KERNEL_HSE, separate_psi=True)
-    phi = synth.random_orbitals(cfg, 41, 3, cuda_device)
-    psi = synth.random_orbitals(cfg, 42, 2, cuda_device)
-    ref = _oracle(cfg, phi, psi)
-    outs = []
-    for env in ({}, {"PTFOCK_SLAB": "legacy"}, {"PTFOCK_PENCIL": "legacy"}):
-        for k in ("PTFOCK_SLAB", "PTFOCK_PENCIL"):
-            monkeypatch.delenv(k, raising=False)
-        for k, v in env.items():
-            monkeypatch.setenv(k, v)
-        with binding.plan_for(cfg, max_targets=2) as plan:
-            out = plan.apply(phi, psi)
-            torch.cuda.synchronize()
-        assert _rel(out.cpu().numpy(), ref) <= TOL, env
-        outs.append(out)

@@ -41,8 +41,9 @@ def test_strerror_and_desc_layout(built_lib):
     assert L.ptfock_strerror(0) == b"ok"
     assert b"no CPU fallback" in L.ptfock_strerror(-3)
     assert L.ptfock_destroy(None) == 0
-    # ptfock_desc: 9 doubles, 3+1+1+1 int32 (+pad), 2 doubles, 3 int32 (+pad), uint64
-    assert ctypes.sizeof(built_lib.Desc) == 72 + 24 + 16 + 16 + 8
+    # ptfock_desc: 9 doubles, 3+1+1+1 int32, 2 doubles, 3 int32 (+pad), uint64, uint32 (+pad)
+    assert ctypes.sizeof(built_lib.Desc) == 72 + 24 + 16 + 16 + 8 + 8
+    assert b"slab shapes" in L.ptfock_strerror(-2)
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
