@@ -215,7 +215,9 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
     peak, peak_src = load_peak()
     N = cfg.N
     Ib, Jb = info1["block_i"], info1["block_j"]
-    if info1.get("pass8"):
+    if info1.get("pass8") == 2:
+        names = ["onchip16_apply (whole pair-solve on chip)", "(no pass B)", "onchip_reduce (sum of the i-chunks)"]
+    elif info1.get("pass8"):
         names = ["p8_fwd (pass A)", "p8_mid (pass B)", "p8_inv_acc (pass C)"]
     else:
         names = ["slabx_fwd / slab_fwd (pass A)", "pencil_tma / pencil_mid (pass B)", "slabx_inv_acc / slab_inv_acc (pass C)"]
@@ -223,6 +225,10 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
     # and writes it (v' amortised over the wave); C reads it, reads phi_i, and read-modify-writes out once per
     # (target, wave).  DESIGN.md 5.
     per_pair = [16.0 * N * (1.0 + 1.0 / Jb + 1.0 / Ib), 32.0 * N, 16.0 * N * (1.0 + 1.0 / Jb + 2.0 / Ib)]
+    if info1.get("pass8") == 2:
+        # on chip: phi_i twice (product, final multiply; the second read hits L1/L2), psi_j and the partial sums once per
+        # CTA; no pair-density traffic at all.  Per pair-solve at most 32 N + (16 N + 32 N) / (orbitals per CTA).
+        per_pair = [32.0 * N + 48.0 * N * max(1, launches // max(1, steps) // 2) / max(1, n_i), 0.0, 0.0]
     tot_ms = max(1e-9, sum(prof["ms"]))
     pairs_prof = pairs_exec * n_prof
     per_kernel = {}
@@ -303,7 +309,8 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
               "kernel": "HSE" if cfg.kernel == 1 else "Coulomb",
               "pair_solves_executed_per_step": pairs_exec, "symmetric_schedule": bool(info1["last_symmetric"]),
               "block_i": Ib, "block_j": Jb, "scratch_bytes": info1["scratch_bytes"],
-              "kernels": "pass8 (two-stage slab passes + 32x32 pencil pass)" if info1.get("pass8") else "three-stage slab passes + pencil pass",
+              "kernels": {0: "three-stage slab passes + pencil pass", 1: "pass8 (two-stage slab passes + 32x32 pencil pass)",
+                          2: "onchip16 (whole pair-solve in one CTA, no scratch)"}[int(info1.get("pass8", 0))],
               "l2": f"inputs + scratch per step = {(16 * N * (n_i + 2 * n_j) + info1['scratch_bytes']) / 1e9:.2f} GB"
                     " (larger than the 126 MB L2; no explicit flush)",
               "parallelism": "replicas only" if world > 1 else "single GPU"}

@@ -30,7 +30,8 @@
  *   (64,64) (128,48) (48,48) (32,32) (90,60)            -- TMA-fed three-stage slab passes
  *   (16,16) (16,32) (32,16) (16,48) (48,32) (32,64)     -- generic slab passes
  * (all BASELINE.json configs, and the paper's own 60 x 90 x 120 grid stored as 120 x 90 x 60).
- * 64 x 64 x 64 additionally has the two-stage slab passes + 32 x 32 pencil pass (the default there).
+ * 64 x 64 x 64 additionally has the two-stage slab passes + 32 x 32 pencil pass, and 16 x 16 x 16 the single-pass
+ * on-chip kernel (whole pair-solve in one CTA, no scratch); both are the default for their grid.
  */
 #ifndef PTFOCK_H
 #define PTFOCK_H
@@ -78,8 +79,9 @@ typedef struct {
 } ptfock_desc;
 
 enum {
-    /* use the three-stage slab passes (slabx.cuh) even where the two-stage passes (pass8.cuh) exist: same
-     * results, kept for A/B timing and as a second implementation the tests compare with the oracle */
+    /* use the three-pass path (slab passes + pencil pass through the pair scratch) even where a grid has a faster
+     * dedicated path (64^3: pass8.cuh, 16^3: onchip16.cuh): same results, kept for A/B timing and as a second
+     * implementation the tests compare with the oracle */
     PTFOCK_FLAG_THREE_STAGE_SLABS = 1u
 };
 
@@ -126,7 +128,8 @@ int ptfock_last_cuda_error(void);
  *   info[0] = block_i, info[1] = block_j in use, info[2] = scratch bytes, info[3] = kernel launches
  *   issued by the most recent apply, info[4] = pair-solves executed by the most recent apply,
  *   info[5] = 1 if the most recent apply used the symmetric schedule, info[6] = total launches since create,
- *   info[7] = 1 if the plan uses the two-stage slab passes + 32 x 32 pencil pass (pass8), else 0. */
+ *   info[7] = kernel family: 0 three-stage slab passes + pencil pass, 1 two-stage slab passes + 32 x 32 pencil pass
+ *             (64^3), 2 single-pass on-chip kernel (16^3). */
 int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]);
 
 /* Test hook: W = IFFT[v' * FFT(conj(phi_i) psi_j)] for ONE pair through the same three kernels,

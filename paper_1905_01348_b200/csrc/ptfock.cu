@@ -6,7 +6,9 @@
 #include "slabx.cuh"
 #include "pencil_tma.cuh"
 #include "pass8.cuh"
+#include "onchip16.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -224,6 +226,7 @@ struct ptfock_plan {
     const struct P8Entry *p8;
     CUtensorMap tmap8;
     double2 *v8_dev;
+    int onchip;                         // 16^3: single-pass on-chip kernel (onchip16.cuh); v_dev then holds v'[k2][k0][k1]
     // optional per-pass device timing (ptfock_set_profiling): events bracket every launch
     int profiling;
     std::vector<cudaEvent_t> *ev_pool;
@@ -266,7 +269,7 @@ void free_plan(ptfock_plan *p) {
 
 // v'(pos0, pos1, pos2) = -alpha/N * v(|G|^2) in the permuted order; also reports whether v(-G) = v(G)
 // holds on the grid (needed by the pair-symmetric schedule; fails for skew cells at Nyquist planes).
-int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, std::vector<double> &vperm, bool &even) {
+int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, bool onchip, std::vector<double> &vperm, bool &even) {
     const int n0 = d.n[0], n1 = d.n[1], n2 = d.n[2];
     const long long N = (long long)n0 * n1 * n2;
     const double *a = d.cell;
@@ -313,6 +316,14 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, s
             }
     const double scale = -d.alpha / (double)N;
     vperm.resize((size_t)N);
+    if (onchip) {
+        // onchip16.cuh: natural frequency order, stored [k2][k0][k1]
+        for (int k0 = 0; k0 < n0; ++k0)
+            for (int k1 = 0; k1 < n1; ++k1)
+                for (int k2 = 0; k2 < n2; ++k2)
+                    vperm[((size_t)k2 * n0 + k0) * n1 + k1] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
+        return PTFOCK_OK;
+    }
     if (p8) {
         // pass8.cuh order: [tile group][m < 16][middle-stage thread t < ntb] pairs (k0b = 2m, 2m + 1), where
         // t = ((k0a*nq + q)*p + pp)*rq + r, k1b = q*rq + r, slab position = group*p + pp = (k2b*a1 + k1a)*a2 + k2a
@@ -391,18 +402,23 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     p->slab = slab;
     p->pencil = pencil;
     p->p8 = p8;
+    p->onchip = (d.n[0] == 16 && d.n[1] == 16 && d.n[2] == 16 && !(d.flags & PTFOCK_FLAG_THREE_STAGE_SLABS)) ? 1 : 0;
     p->sm_count = prop.multiProcessorCount;
 
     std::vector<double> vperm;
     bool even = false;
-    int rc = build_vtable(d, *slab, p8, vperm, even);
+    int rc = build_vtable(d, *slab, p8, p->onchip != 0, vperm, even);
     if (rc != PTFOCK_OK) { free_plan(p); return rc; }
     p->v_even = even;
 
 #define CUP(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_cuda = (int)e__; free_plan(p); \
         return (e__ == cudaErrorMemoryAllocation) ? PTFOCK_ERR_ALLOC : PTFOCK_ERR_CUDA; } } while (0)
 
-    if (p8) {
+    if (p->onchip) {
+        CUP(cudaFuncSetAttribute(onchip16_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, kOnchipSmem));
+        CUP(cudaMalloc(&p->v_dev, sizeof(double) * p->N));
+        CUP(cudaMemcpy(p->v_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
+    } else if (p8) {
         CUP(p8->prepare());
         CUP(cudaMalloc(&p->v8_dev, sizeof(double) * p->N));
         CUP(cudaMemcpy(p->v8_dev, vperm.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice));
@@ -547,7 +563,7 @@ extern "C" int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]) {
     info[4] = plan->last_pairs;
     info[5] = plan->last_symmetric;
     info[6] = plan->total_launches;
-    info[7] = plan->p8 ? 1 : 0;
+    info[7] = plan->onchip ? 2 : (plan->p8 ? 1 : 0);
     return PTFOCK_OK;
 }
 
@@ -695,16 +711,58 @@ struct HostPipe {
     }
 };
 
+// 16^3: out[j] = sum_i mul_i * W_ij with the whole pair-solve inside one CTA (onchip16.cuh); the i loop is split into
+// chunks so that the grid fills the SMs, the chunks' partial sums go through the plan's scratch and are added in order
+int apply_onchip(ptfock_plan *p, const cd *phi, const cd *mul, int mul_stride, int phi0, int n_i, const cd *tgt, int n_targets,
+                 cd *out, cudaStream_t st, Wave &w) {
+    const size_t gbytes = sizeof(cd) * (size_t)p->N;
+    const int max_batch = (int)std::min<size_t>(p->scratch_bytes / gbytes, 65535);
+    for (int t0 = 0; t0 < n_targets; t0 += max_batch) {
+        const int nt = std::min(max_batch, n_targets - t0);
+        int n_chunks = (2 * p->sm_count + nt - 1) / nt;
+        n_chunks = std::max(1, std::min(n_chunks, n_i));
+        n_chunks = (int)std::min<size_t>((size_t)n_chunks, p->scratch_bytes / (gbytes * nt));
+        n_chunks = std::min(n_chunks, 65535);
+        const int per = (n_i + n_chunks - 1) / n_chunks;
+        n_chunks = (n_i + per - 1) / per;
+        OnchipArgs a;
+        a.phi = phi; a.mul = mul; a.psi = tgt; a.partial = p->scratch; a.vt = p->v_dev;
+        a.phi0 = phi0; a.n_i = n_i; a.mul_stride = mul_stride; a.psi0 = t0; a.i_per_cta = per;
+        mark(w, -1);
+        onchip16_apply<<<dim3(nt, n_chunks), kOnchipThreads, kOnchipSmem, st>>>(a);
+        mark(w, 0);
+        const long long per_chunk = (long long)nt * p->N;
+        onchip_reduce<<<(unsigned)((per_chunk + 255) / 256), 256, 0, st>>>(p->scratch, n_chunks, per_chunk, out + (size_t)t0 * p->N);
+        mark(w, 2);
+        w.launches += 2;
+        w.pairs += (long long)n_i * nt;
+        w.note(cudaPeekAtLastError());
+    }
+    return PTFOCK_OK;
+}
+
 int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, int n_targets, cd *out,
                  cudaStream_t st, HostPipe *hp = nullptr) {
     const size_t gbytes = sizeof(cd) * (size_t)p->N;
     if (n_targets == 0) { p->last_launches = 0; p->last_pairs = 0; p->last_symmetric = 0; return PTFOCK_OK; }
     if (overlaps(out, gbytes * n_targets, phi, gbytes * p->d.n_occ)) return PTFOCK_ERR_ALIAS;
     if (psi && overlaps(out, gbytes * n_targets, psi, gbytes * n_targets)) return PTFOCK_ERR_ALIAS;
-    CU(cudaMemsetAsync(out, 0, gbytes * n_targets, st));             // Alg. 2 line 1
     Wave w{ p, st, 0, 0, cudaSuccess };
     const int n_occ = p->d.n_occ;
-    const bool symmetric = (!psi) && self_offset == 0 && n_targets == n_occ && p->v_even && n_occ > 1;
+    const bool symmetric = (!psi) && self_offset == 0 && n_targets == n_occ && p->v_even && n_occ > 1 && !p->onchip;
+    if (p->onchip) {
+        if (hp) { hp->need(st, 0, n_occ); if (psi) w.note(cudaStreamWaitEvent(st, (*hp->ev)[hp->n_chunks], 0)); }
+        apply_onchip(p, phi, phi, 1, 0, n_occ, psi ? psi : phi + (size_t)self_offset * p->N, n_targets, out, st, w);
+        if (hp) w.note(hp->err);
+        w.note(cudaGetLastError());
+        if (w.err != cudaSuccess) { g_last_cuda = (int)w.err; return PTFOCK_ERR_CUDA; }
+        p->last_launches = w.launches;
+        p->last_pairs = w.pairs;
+        p->last_symmetric = 0;
+        p->total_launches += w.launches;
+        return PTFOCK_OK;
+    }
+    CU(cudaMemsetAsync(out, 0, gbytes * n_targets, st));             // Alg. 2 line 1
     if (symmetric) {
         // square blocks; block pair (bi <= bj): W_ij for i in bi, j in bj serves out_j (as is) and, off the
         // diagonal, out_i through W_ji = conj(W_ij) (v real and even).
@@ -881,10 +939,14 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
         if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
         fill_ones<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(plan->ones, plan->N);
     }
-    CU(cudaMemsetAsync(w_out, 0, gbytes, st));
     Wave w{ plan, st, 0, 0, cudaSuccess };
-    wave_forward_mid(w, (const cd *)phi_i, (const cd *)psi_j, 0, 1, 0, 1);
-    wave_accumulate(w, plan->ones, 0, 1, (cd *)w_out, 0, 1, 1, 1, 0);
+    if (plan->onchip) {
+        apply_onchip(plan, (const cd *)phi_i, plan->ones, 0, 0, 1, (const cd *)psi_j, 1, (cd *)w_out, st, w);
+    } else {
+        CU(cudaMemsetAsync(w_out, 0, gbytes, st));
+        wave_forward_mid(w, (const cd *)phi_i, (const cd *)psi_j, 0, 1, 0, 1);
+        wave_accumulate(w, plan->ones, 0, 1, (cd *)w_out, 0, 1, 1, 1, 0);
+    }
     plan->total_launches += w.launches + 1;
     w.note(cudaGetLastError());
     if (w.err != cudaSuccess) { g_last_cuda = (int)w.err; return PTFOCK_ERR_CUDA; }

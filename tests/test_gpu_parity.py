@@ -25,7 +25,7 @@ def _oracle(cfg, phi, psi=None, cols=None):
 
 SMALL = [
     # name, edges, grid, n_occ, kernel, separate psi
-    ("c16", (10.26,) * 3, (16, 16, 16), 5, synth.KERNEL_HSE, False),
+    ("c16", (10.26,) * 3, (16, 16, 16), 5, synth.KERNEL_HSE, False),          # three-pass path (the flag below)
     ("c16ns", (10.26,) * 3, (16, 16, 16), 5, synth.KERNEL_COULOMB, True),
     ("g16x32x16", (9.0, 17.0, 12.0), (16, 32, 16), 4, synth.KERNEL_HSE, True),
     ("g32x16x32", (15.0, 9.0, 17.0), (32, 16, 32), 3, synth.KERNEL_COULOMB, False),
@@ -45,7 +45,7 @@ def test_small_grids_every_codelet(cuda_device, case):
     cfg = synth.Config(name, edges, n, n_occ, kernel, separate_psi=sep)
     phi = synth.random_orbitals(cfg, 11, n_occ, cuda_device)
     psi = synth.random_orbitals(cfg, 12, 3, cuda_device) if sep else None
-    with binding.plan_for(cfg, block_i=2, block_j=2) as plan:
+    with binding.plan_for(cfg, block_i=2, block_j=2, flags=binding.FLAG_THREE_STAGE_SLABS) as plan:
         out = plan.apply(phi, psi)
         torch.cuda.synchronize()
     assert _rel(out.cpu().numpy(), _oracle(cfg, phi, psi)) <= TOL
@@ -61,14 +61,15 @@ def test_debug_pair_matches_oracle_W(cuda_device):
 
 
 def test_Si8_full(cuda_device):
+    """Si8 through the three-pass path (symmetric schedule); the default on-chip kernel: tests/test_gpu_onchip16.py."""
     cfg = synth.CONFIGS["Si8"]
     phi = synth.orbitals(cfg, device=cuda_device)
-    with binding.plan_for(cfg) as plan:
+    with binding.plan_for(cfg, flags=binding.FLAG_THREE_STAGE_SLABS) as plan:
         out = plan.apply(phi)
         e = plan.exchange_energy(phi, vx_psi=out)
         e2 = plan.exchange_energy(phi)
         info = plan.info()
-    assert info["last_symmetric"] == 1
+    assert info["last_symmetric"] == 1 and info["pass8"] == 0
     ref = _oracle(cfg, phi)
     assert _rel(out.cpu().numpy(), ref) <= TOL
     e_ref = oracle.exchange_energy(cfg.cell, cfg.n, phi.cpu().numpy(), ref)
@@ -119,7 +120,7 @@ def test_host_path_and_stream(cuda_device):
     cfg2 = synth.Config("h2", (10.26,) * 3, (16, 16, 16), 7, synth.KERNEL_COULOMB)
     phi2 = synth.random_orbitals(cfg2, 3, 7, cuda_device)
     hphi = phi2.cpu().pin_memory()
-    with binding.plan_for(cfg2, block_i=2, block_j=2) as plan:
+    with binding.plan_for(cfg2, block_i=2, block_j=2, flags=binding.FLAG_THREE_STAGE_SLABS) as plan:
         for off, nt in ((0, 7), (5, 2), (1, 5)):
             dev = plan.apply(phi2, None, self_offset=off, n_targets=nt)
             sym = plan.info()["last_symmetric"]
@@ -167,7 +168,7 @@ def test_oversized_tile_is_clamped(cuda_device):
     cfg = synth.Config("big", (10.26,) * 3, (16, 16, 16), 300, synth.KERNEL_HSE, separate_psi=True)
     phi = synth.random_orbitals(cfg, 7, 300, cuda_device)
     psi = synth.random_orbitals(cfg, 8, 300, cuda_device)
-    with binding.plan_for(cfg, block_i=300, block_j=300) as plan:
+    with binding.plan_for(cfg, block_i=300, block_j=300, flags=binding.FLAG_THREE_STAGE_SLABS) as plan:
         info = plan.info()
         assert info["block_i"] * info["block_j"] <= 65535
         out = plan.apply(phi, psi)
@@ -182,7 +183,7 @@ def test_symmetric_blocks_stay_launchable(cuda_device):
     block^2 pair-solves exceed what one launch can index."""
     cfg = synth.Config("sym512", (10.26,) * 3, (16, 16, 16), 512, synth.KERNEL_COULOMB)
     phi = synth.random_orbitals(cfg, 9, 512, cuda_device)
-    with binding.plan_for(cfg) as plan:
+    with binding.plan_for(cfg, flags=binding.FLAG_THREE_STAGE_SLABS) as plan:
         out = plan.apply(phi)
         torch.cuda.synchronize()
         assert plan.info()["last_symmetric"] == 1
