@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ptfock_ref.c")
+_SRC_DENSE = os.path.join(_HERE, "ptdense_ref.c")       # dense-algebra neighbours (Alg. 3, Sec. 3.4)
 _LIB = os.path.join(_HERE, "libptfock_ref.so")
 
 KERNEL_COULOMB = 0
@@ -25,8 +26,9 @@ KERNEL_HSE = 1
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (-O2 -fopenmp, no fast-math).  Returns the path of the .so."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c99", "-o", _LIB, _SRC, "-lm"]
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_DENSE))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
+        cmd = ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c99", "-o", _LIB, _SRC, _SRC_DENSE, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -55,6 +57,15 @@ def lib() -> ctypes.CDLL:
         _lib.ptfock_ref_dft1d_naive.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp]
         _lib.ptfock_ref_dft1d_naive.restype = None
         _lib.ptfock_ref_num_threads.restype = ctypes.c_int
+        i64, i32, f64 = ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+        _lib.ptdense_ref_overlap.argtypes = [i64, f64, dp, i32, dp, i32, dp]
+        _lib.ptdense_ref_rotate.argtypes = [i64, dp, i32, dp, i32, dp]
+        _lib.ptdense_ref_residual.argtypes = [i64, f64, i32, f64, dp, dp, dp, dp]
+        _lib.ptdense_ref_density.argtypes = [i64, dp, i32, dp]
+        _lib.ptdense_ref_cholesky.argtypes = [i32, dp, dp]
+        _lib.ptdense_ref_orthonormalize.argtypes = [i64, f64, dp, i32, dp]
+        for f in ("overlap", "rotate", "residual", "density", "cholesky", "orthonormalize"):
+            getattr(_lib, "ptdense_ref_" + f).restype = ctypes.c_int
     return _lib
 
 
@@ -172,3 +183,88 @@ def dft1d_naive(x: np.ndarray, sign: int) -> np.ndarray:
     y = np.empty_like(x)
     lib().ptfock_ref_dft1d_naive(int(x.size), int(sign), _ptr(x), _ptr(y))
     return y
+
+
+# ---- dense-algebra neighbours (oracle/ptdense_ref.c; Alg. 3, Sec. 3.4) ---------------
+def _orbs(a, what: str):
+    a = _c128(a, what)
+    if a.ndim < 2:
+        raise ValueError(f"{what} must be [n_orbitals, points...]")
+    return a, a.shape[0], a.size // max(1, a.shape[0])
+
+
+def overlap(a: np.ndarray, b: np.ndarray, weight: float) -> np.ndarray:
+    """S[m, n] = weight * sum_r conj(a_m(r)) b_n(r)."""
+    a, n_a, N = _orbs(a, "a")
+    b, n_b, Nb = _orbs(b, "b")
+    if N != Nb:
+        raise ValueError("a and b live on different grids")
+    s = np.empty((n_a, n_b), dtype=np.complex128)
+    rc = lib().ptdense_ref_overlap(N, float(weight), _ptr(a), n_a, _ptr(b), n_b, _ptr(s))
+    if rc != 0:
+        raise RuntimeError(f"ptdense_ref_overlap failed: {rc}")
+    return s
+
+
+def rotate(a: np.ndarray, s: np.ndarray) -> np.ndarray:
+    """out_n(r) = sum_m a_m(r) S[m, n]."""
+    a, n_a, N = _orbs(a, "a")
+    s = _c128(s, "s")
+    if s.ndim != 2 or s.shape[0] != n_a:
+        raise ValueError("S must be [n_a, n_out]")
+    out = np.empty((s.shape[1],) + a.shape[1:], dtype=np.complex128)
+    rc = lib().ptdense_ref_rotate(N, _ptr(a), n_a, _ptr(s), s.shape[1], _ptr(out))
+    if rc != 0:
+        raise RuntimeError(f"ptdense_ref_rotate failed: {rc}")
+    return out
+
+
+def residual(psi: np.ndarray, hpsi: np.ndarray, weight: float, dt: float = 0.0, psi_half: np.ndarray | None = None) -> np.ndarray:
+    """psi_half None: R_n = H Psi - Psi (Psi^* H Psi); else R_f = Psi + (i dt/2)(H Psi - Psi (Psi^* H Psi)) - Psi_half."""
+    psi, n, N = _orbs(psi, "psi")
+    hpsi = _c128(hpsi, "hpsi")
+    if hpsi.shape != psi.shape:
+        raise ValueError("hpsi must have psi's shape")
+    half_p = ctypes.c_void_p(0)
+    if psi_half is not None:
+        psi_half = _c128(psi_half, "psi_half")
+        if psi_half.shape != psi.shape:
+            raise ValueError("psi_half must have psi's shape")
+        half_p = _ptr(psi_half)
+    r = np.empty_like(psi)
+    rc = lib().ptdense_ref_residual(N, float(weight), n, float(dt), _ptr(psi), _ptr(hpsi), half_p, _ptr(r))
+    if rc != 0:
+        raise RuntimeError(f"ptdense_ref_residual failed: {rc}")
+    return r
+
+
+def density(psi: np.ndarray) -> np.ndarray:
+    """rho(r) = sum_i |psi_i(r)|^2 (shape of one grid)."""
+    psi, n, N = _orbs(psi, "psi")
+    rho = np.empty(psi.shape[1:], dtype=np.float64)
+    rc = lib().ptdense_ref_density(N, _ptr(psi), n, _ptr(rho))
+    if rc != 0:
+        raise RuntimeError(f"ptdense_ref_density failed: {rc}")
+    return rho
+
+
+def cholesky(s: np.ndarray) -> np.ndarray:
+    """Lower-triangular L with S = L L^H (S Hermitian positive definite)."""
+    s = _c128(s, "s")
+    if s.ndim != 2 or s.shape[0] != s.shape[1]:
+        raise ValueError("S must be square")
+    l = np.empty_like(s)
+    rc = lib().ptdense_ref_cholesky(s.shape[0], _ptr(s), _ptr(l))
+    if rc != 0:
+        raise RuntimeError(f"ptdense_ref_cholesky failed: {rc}")
+    return l
+
+
+def orthonormalize(psi: np.ndarray, weight: float) -> np.ndarray:
+    """Psi L^{-H} with L L^H = Psi^* Psi (Cholesky + triangular solve)."""
+    psi, n, N = _orbs(psi, "psi")
+    out = np.empty_like(psi)
+    rc = lib().ptdense_ref_orthonormalize(N, float(weight), _ptr(psi), n, _ptr(out))
+    if rc != 0:
+        raise RuntimeError(f"ptdense_ref_orthonormalize failed: {rc}")
+    return out
