@@ -322,6 +322,64 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
             "vs_baseline": (value / world / PAPER_PAIRS_PER_S[cfg.name]) if cfg.name in PAPER_PAIRS_PER_S else None}
 
 
+def dense_leg(cfg, args, dev, local):
+    """--leg dense: the dense-algebra neighbours (Alg. 3, Sec. 3.4) at cfg's sizes, each
+    timed alone with CUDA events on the launching stream; roofline = the plain FP64 pipe (measured live) for the
+    contractions, HBM for the density."""
+    import torch
+    from paper_1905_01348_b200 import binding, synth
+    n = cfg.j_block * 8 if cfg.j_block else cfg.n_occ          # Si1536: 768 orbitals keep the run inside a minute
+    psi = synth.orbitals(cfg, cfg.seed_phi, n, dev)
+    g = torch.Generator(device="cpu").manual_seed(5)
+    hpsi = psi * 0.5 + 0.1 * torch.roll(psi, 1, 0)
+    half = torch.roll(psi, 2, 0).contiguous()
+    N = cfg.N
+    peak_hbm, _ = load_peak()
+    p64 = binding.measure_fp64_peak(local)
+    out = {}
+    with binding.Plan(cfg.cell, cfg.n, n, n, cfg.kernel, cfg.omega, cfg.alpha, local) as plan:
+        s = torch.empty((n, n), dtype=torch.complex128, device=dev)
+        r = torch.empty_like(psi)
+        rho = torch.empty(cfg.n, dtype=torch.float64, device=dev)
+        mix = (psi + 0.05 * torch.roll(psi, 1, 0)).contiguous()
+        work = mix.clone()
+
+        def timed(fn, reps, setup=None):
+            ts = []
+            for k in range(reps + 1):
+                if setup:
+                    setup()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                fn()
+                e1.record()
+                torch.cuda.synchronize()
+                if k:
+                    ts.append(e0.elapsed_time(e1))
+            return statistics.median(ts)
+
+        legs = {
+            "overlap (Alg. 3 line 2)": (lambda: plan.overlap(psi, hpsi, out=s), None, 8.0 * N * n * n, 32.0 * N * n),
+            "residual R_f (Alg. 3 lines 2-5)": (lambda: plan.residual(psi, hpsi, dt=0.5, psi_half=half, out=r), None,
+                                                16.0 * N * n * n, 80.0 * N * n),
+            "density (Sec. 3.4)": (lambda: plan.density(psi, out=rho), None, 4.0 * N * n, 16.0 * N * n),
+            "orthonormalize (Sec. 3.4: overlap + Cholesky + Trsm)": (lambda: plan.orthonormalize(work), lambda: work.copy_(mix),
+                                                                    12.0 * N * n * n + 4.0 / 3.0 * n ** 3, 48.0 * N * n),
+        }
+        for name, (fn, setup, flops, byts) in legs.items():
+            ms = timed(fn, args.steps, setup)
+            tf, gbs = flops / (ms * 1e-3) / 1e12, byts / (ms * 1e-3) / 1e9
+            bound = "hbm" if name.startswith("density") else "alu"
+            out[name] = {"ms": ms, "TFLOP/s": tf, "GB/s": gbs, "bound": bound,
+                         "frac": gbs / peak_hbm if bound == "hbm" else tf / p64}
+    line = {"metric": "dense-algebra neighbours of the Fock exchange path (fp64, 1 B200)", "unit": "ms per call",
+            "config": {"workload": f"{cfg.name}: {n} orbitals on {'x'.join(map(str, cfg.n))}", "leg": "dense"},
+            "dtype": "f64", "data": "synthetic", "steps": args.steps,
+            "roofline": {"alu_peak_tflops": p64, "alu_peak_source": "measured live (ptfock_measure_dfma_peak)",
+                         "hbm_peak_gbs": peak_hbm, "per_call": out}}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -339,6 +397,8 @@ def main():
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the second headline config (one Si1536 j-block) that the default Si512 run also times")
     ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")
+    ap.add_argument("--leg", default="fock", choices=["fock", "dense"],
+                    help="fock: the headline exchange path (default); dense: the dense-algebra neighbours, own JSON line")
     args = ap.parse_args()
 
     from paper_1905_01348_b200 import synth
@@ -363,6 +423,12 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     binding.lib()                                   # fails loudly if the CUDA library is missing
+    if args.leg == "dense":
+        if rank == 0:
+            dense_leg(cfg, args, dev, local)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     m = measure(cfg, args, dev, local, rank, world, args.steps, args.warmup, not args.no_e2e, not args.no_cpu, args.check)
     # the north-star target names Si512 AND Si1536: the default run also times one streamed j-block of Si1536
     # (bounded: 2 warm-up + 3 timed steps, no e2e / CPU legs) and reports it under config.secondary / roofline.by_config

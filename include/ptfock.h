@@ -58,7 +58,8 @@ enum {
     PTFOCK_ERR_ALIGNMENT = -4,          /* an orbital pointer is not 16-byte aligned */
     PTFOCK_ERR_ALLOC = -5,              /* device or host allocation failed (workspace too small included) */
     PTFOCK_ERR_CUDA = -6,               /* a CUDA runtime call failed; see ptfock_last_cuda_error */
-    PTFOCK_ERR_ALIAS = -7               /* out overlaps phi or psi */
+    PTFOCK_ERR_ALIAS = -7,              /* out overlaps phi or psi */
+    PTFOCK_ERR_NOT_POSITIVE = -8        /* ptfock_orthonormalize: the overlap matrix is not positive definite */
 };
 
 typedef struct {
@@ -114,6 +115,36 @@ int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const void *psi, 
  * n_targets <= max_targets. */
 int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const void *psi_host, int32_t self_offset,
                       int32_t n_targets, void *out_host, void *stream);
+
+/* ---- dense-algebra neighbours of the exchange operator ------------------------------------
+ * The steps either side of H Psi in one PT-CN step (Alg. 1): the residuals of PAPER.md:171-188
+ * (Sec. 3.3, Alg. 3), the density of PAPER.md:192 and the re-orthogonalisation of PAPER.md:200 (Sec. 3.4), on ONE GPU
+ * (the paper's Alltoallv / Allreduce steps, Alg. 3 lines 1, 3, 6, have nothing to do here).  Orbital sets are
+ * [orbital][x0][x1][x2] complex fp64 DEVICE arrays on the plan's grid; (a, b) = (Omega/N) sum_r conj(a(r)) b(r).
+ * Matrices are row-major complex fp64 DEVICE arrays.  All calls are asynchronous on `stream` except where stated,
+ * use the plan's scratch (PTFOCK_ERR_ALLOC if it is too small) and are deterministic (no atomics). */
+
+/* S[m][n] = (a_m, b_n), m < n_a, n < n_b (Alg. 3 line 2: "S = Psi_f^* H_f Psi_f"; "Psi^* Psi"). */
+int ptfock_overlap(ptfock_plan *plan, const void *a, int32_t n_a, const void *b, int32_t n_b, void *s, void *stream);
+
+/* out_n(r) = sum_m a_m(r) S[m][n], n < n_out; S is n_a x n_out (Alg. 3 line 4: "Psi_temp = Psi_f S").  out must not
+ * overlap a. */
+int ptfock_rotate(ptfock_plan *plan, const void *a, int32_t n_a, const void *s, int32_t n_out, void *out, void *stream);
+
+/* psi_half == NULL:  R = H Psi - Psi (Psi^* H Psi)                                   (Alg. 1 line 1, R_n)
+ * else:              R = Psi + (i dt/2) (H Psi - Psi (Psi^* H Psi)) - Psi_half       (Alg. 3 line 5, R_f; the minus signs
+ *                    the extraction of PAPER.md dropped are those of Eq. (5))
+ * psi, hpsi, psi_half, r_out: n orbitals each; r_out must not overlap psi. */
+int ptfock_residual(ptfock_plan *plan, const void *psi, const void *hpsi, const void *psi_half, int32_t n, double dt,
+                    void *r_out, void *stream);
+
+/* rho(r) = sum_{i<n} |psi_i(r)|^2; rho: N doubles, DEVICE. */
+int ptfock_density(ptfock_plan *plan, const void *psi, int32_t n, double *rho, void *stream);
+
+/* Psi <- Psi L^{-H} with L L^H = Psi^* Psi (overlap, Cholesky, triangular solve), IN PLACE; afterwards
+ * (psi_m, psi_n) = delta_mn.  Synchronises `stream`; PTFOCK_ERR_NOT_POSITIVE if a pivot is not positive (psi is then
+ * left modified). */
+int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, void *stream);
 
 /* Frees everything the plan owns.  NULL is allowed. */
 int ptfock_destroy(ptfock_plan *plan);

@@ -21,7 +21,8 @@ FLAG_THREE_STAGE_SLABS = 1
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
-           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_copy_bandwidth"]
+           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_copy_bandwidth",
+           "ptfock_overlap", "ptfock_rotate", "ptfock_residual", "ptfock_density", "ptfock_orthonormalize"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "1886"]
@@ -79,6 +80,11 @@ def lib() -> ctypes.CDLL:
         L.ptfock_get_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64), i32]
         L.ptfock_measure_dfma_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double)]
         L.ptfock_measure_copy_bandwidth.argtypes = [i32, ctypes.c_uint64, i32, ctypes.POINTER(ctypes.c_double)]
+        L.ptfock_overlap.argtypes = [vp, vp, i32, vp, i32, vp, vp]
+        L.ptfock_rotate.argtypes = [vp, vp, i32, vp, i32, vp, vp]
+        L.ptfock_residual.argtypes = [vp, vp, vp, vp, i32, ctypes.c_double, vp, vp]
+        L.ptfock_density.argtypes = [vp, vp, i32, vp, vp]
+        L.ptfock_orthonormalize.argtypes = [vp, vp, i32, vp]
         for name in EXPORTS:
             if name != "ptfock_strerror":
                 getattr(L, name).restype = ctypes.c_int
@@ -201,6 +207,64 @@ class Plan:
                                        _dev_ptr(psi_j, "psi_j", self.device), _dev_ptr(w, "w", self.device),
                                        _stream(self.device)), "ptfock_debug_pair")
         return w
+
+    # ---- dense-algebra neighbours (Alg. 3, Sec. 3.4) ----------------------------------------------------
+    def _mat_ptr(self, t, what):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()):
+            raise TypeError(f"{what} must be a contiguous complex128 CUDA tensor")
+        if t.device.index != self.device:
+            raise ValueError(f"{what} is on {t.device}, the plan is on cuda:{self.device}")
+        return ctypes.c_void_p(t.data_ptr())
+
+    def overlap(self, a, b, out=None):
+        """S[m, n] = (Omega/N) sum_r conj(a_m(r)) b_n(r)."""
+        import torch
+        n_a, n_b = self._grids(a, "a"), self._grids(b, "b")
+        if out is None:
+            out = torch.empty((n_a, n_b), dtype=torch.complex128, device=a.device)
+        _check(lib().ptfock_overlap(self._h, _dev_ptr(a, "a", self.device), n_a, _dev_ptr(b, "b", self.device), n_b,
+                                    self._mat_ptr(out, "out"), _stream(self.device)), "ptfock_overlap")
+        return out
+
+    def rotate(self, a, s, out=None):
+        """out_n = sum_m a_m S[m, n]."""
+        import torch
+        n_a = self._grids(a, "a")
+        if s.shape[0] != n_a:
+            raise ValueError("S must be [n_a, n_out]")
+        if out is None:
+            out = torch.empty((s.shape[1],) + self.n, dtype=torch.complex128, device=a.device)
+        _check(lib().ptfock_rotate(self._h, _dev_ptr(a, "a", self.device), n_a, self._mat_ptr(s, "s"), int(s.shape[1]),
+                                   _dev_ptr(out, "out", self.device), _stream(self.device)), "ptfock_rotate")
+        return out
+
+    def residual(self, psi, hpsi, dt: float = 0.0, psi_half=None, out=None):
+        """psi_half None: H psi - psi (psi^* H psi); else psi + (i dt/2)(H psi - psi (psi^* H psi)) - psi_half."""
+        import torch
+        n = self._grids(psi, "psi")
+        if out is None:
+            out = torch.empty_like(psi)
+        _check(lib().ptfock_residual(self._h, _dev_ptr(psi, "psi", self.device), _dev_ptr(hpsi, "hpsi", self.device),
+                                     _dev_ptr(psi_half, "psi_half", self.device), n, float(dt),
+                                     _dev_ptr(out, "out", self.device), _stream(self.device)), "ptfock_residual")
+        return out
+
+    def density(self, psi, out=None):
+        import torch
+        n = self._grids(psi, "psi")
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float64, device=psi.device)
+        _check(lib().ptfock_density(self._h, _dev_ptr(psi, "psi", self.device), n, ctypes.c_void_p(out.data_ptr()),
+                                    _stream(self.device)), "ptfock_density")
+        return out
+
+    def orthonormalize(self, psi):
+        """In place: psi <- psi L^{-H}, L L^H = psi^* psi."""
+        n = self._grids(psi, "psi")
+        _check(lib().ptfock_orthonormalize(self._h, _dev_ptr(psi, "psi", self.device), n, _stream(self.device)),
+               "ptfock_orthonormalize")
+        return psi
 
     def info(self) -> dict:
         a = (ctypes.c_int64 * 8)()

@@ -1,0 +1,346 @@
+// dense.cuh -- the dense-algebra neighbours of the Fock exchange path on one GPU:
+// overlap matrices, rotations, the PT-CN residuals, the density, Cholesky + triangular solve orthonormalisation
+// (Sec. 3.3 Alg. 3; Sec. 3.4).  The paper calls cuBLAS / cuSOLVER for these; here they
+// are hand-written fp64 kernels on the plain FP64 pipe (register-tiled, shared-memory staged), all deterministic
+// (split-K partial sums are added in a fixed order, no atomics).
+//
+// Orbitals are [orbital][grid point] complex fp64, the inner product is (a, b) = w sum_r conj(a(r)) b(r), w = Omega/N.
+#pragma once
+#include "codelets.cuh"
+
+namespace ptfock {
+
+constexpr int kDT = 64;         // output tile edge of the GEMM-like kernels (16 x 16 threads, 4 x 4 complex per thread)
+constexpr int kDK = 16;         // contraction step staged through shared memory
+constexpr int kDP = kDK + 1;    // pitch of a [64][16] tile (elements)
+
+// ---- overlap: part[ks][m][n] = sum over this split's points of conj(a[m][r]) b[n][r] -----------------------------------
+// grid = (ceil(n_a / 64), ceil(n_b / 64), k_splits); thread (ty, tx) owns rows m = ty + 16 i and columns n = tx + 16 j:
+// the shared-memory reads of a tile are a broadcast (a) or 16 consecutive pitch-17 rows (b): conflict free.
+struct OverlapArgs {
+    const cd *a, *b;
+    cd *part;               // [k_splits][n_a_pad? no: n_a][ld]
+    long long n_pts, pts_per_split;
+    int n_a, n_b, ld;       // ld = row pitch of part / S (>= n_b)
+};
+
+__global__ void __launch_bounds__(256) overlap_partial(const OverlapArgs g) {
+    __shared__ cd As[kDT * kDP], Bs[kDT * kDP];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int m0 = blockIdx.x * kDT, n0 = blockIdx.y * kDT;
+    const long long r_beg = (long long)blockIdx.z * g.pts_per_split;
+    const long long r_end = min(g.n_pts, r_beg + g.pts_per_split);
+    cd acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
+    // loader: thread t brings points 4 (t % 4) .. + 3 of row t / 4 of both tiles
+    const int lrow = tid >> 2, lk = (tid & 3) * 4;
+    const bool a_ok = m0 + lrow < g.n_a, b_ok = n0 + lrow < g.n_b;
+    const cd *ap = g.a + (long long)(m0 + lrow) * g.n_pts + lk;
+    const cd *bp = g.b + (long long)(n0 + lrow) * g.n_pts + lk;
+    for (long long r = r_beg; r < r_end; r += kDK) {
+        cd av[4], bv[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const bool in = r + lk + q < r_end;
+            av[q] = (a_ok && in) ? ap[r + q] : make_double2(0.0, 0.0);
+            bv[q] = (b_ok && in) ? bp[r + q] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();                                // the previous step's reads are done
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { As[lrow * kDP + lk + q] = av[q]; Bs[lrow * kDP + lk + q] = bv[q]; }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < kDK; ++kk) {
+            cd x[4], y[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) x[i] = As[(ty + 16 * i) * kDP + kk];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) y[j] = Bs[(tx + 16 * j) * kDP + kk];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {           // acc += conj(x) y
+                    acc[i][j].x = fma(x[i].x, y[j].x, fma(x[i].y, y[j].y, acc[i][j].x));
+                    acc[i][j].y = fma(x[i].x, y[j].y, fma(-x[i].y, y[j].x, acc[i][j].y));
+                }
+        }
+    }
+    cd *out = g.part + (long long)blockIdx.z * g.n_a * g.ld;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int m = m0 + ty + 16 * i, n = n0 + tx + 16 * j;
+            if (m < g.n_a && n < g.n_b) out[(long long)m * g.ld + n] = acc[i][j];
+        }
+}
+
+// s[m][n] = w * sum_ks part[ks][m][n] (fixed order)
+__global__ void __launch_bounds__(256) overlap_reduce(const cd *part, int k_splits, int n_a, int n_b, int ld_part, double w,
+                                                      cd *s, int ld_s) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= (long long)n_a * n_b) return;
+    const int m = (int)(k / n_b), n = (int)(k % n_b);
+    cd t = part[(long long)m * ld_part + n];
+    for (int q = 1; q < k_splits; ++q) {
+        const cd u = part[((long long)q * n_a + m) * ld_part + n];
+        t.x += u.x; t.y += u.y;
+    }
+    s[(long long)m * ld_s + n] = make_double2(t.x * w, t.y * w);
+}
+
+// ---- rotation with fused epilogues: acc_n(r) = sum_m a_m(r) c(m, n) ---------------------------------------------------
+// c(m, n) = S[m*ld + n]  or, for the triangular solve, conj(S[n*ld + m]);
+// mode 0: out = acc                      (Alg. 3 line 4, Psi_temp = Psi_f S)
+// mode 1: out = h - acc                  (Alg. 1 line 1, R_n = H Psi - Psi S)
+// mode 2: out = p + f (h - acc) - q      (Alg. 3 line 5, R_f; f = i dt / 2)
+// mode 3: out = out - acc                (blocked triangular solve: block column minus the finished columns' part)
+// grid = (ceil(n_pts / 64), ceil(n_out / 64)); thread (ty, tx) owns columns n = ty + 16 i and points r = tx + 16 j.
+struct RotateArgs {
+    const cd *a;            // [n_a][n_pts]
+    const cd *s;            // coefficients
+    const cd *h, *p, *q;    // epilogue operands, [n_out][n_pts]
+    cd *out;                // [n_out][n_pts]
+    long long n_pts;
+    int n_a, n_out, ld, conj_t, mode;
+    int n_first;            // first output column (offset into h, p, q, out and into S's column index)
+    double fx, fy;          // f
+};
+
+__global__ void __launch_bounds__(256) rotate_kernel(const RotateArgs g) {
+    __shared__ cd As[kDK * kDT], Ss[kDK * (kDT + 1)];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const long long r0 = (long long)blockIdx.x * kDT;
+    const int n0 = g.n_first + blockIdx.y * kDT, n_end = g.n_first + g.n_out;
+    cd acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
+    // loaders: A tile [16 m][64 r]: thread t -> m = t / 16, r = 4 (t % 16) .. + 3;  S tile [16 m][64 n] likewise
+    const int lm = tid >> 4, lc = (tid & 15) * 4;
+    for (int m0 = 0; m0 < g.n_a; m0 += kDK) {
+        cd av[4], sv[4];
+        const bool m_ok = m0 + lm < g.n_a;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            av[q] = (m_ok && r0 + lc + q < g.n_pts) ? g.a[(long long)(m0 + lm) * g.n_pts + r0 + lc + q] : make_double2(0.0, 0.0);
+            const int n = n0 + lc + q;
+            if (m_ok && n < n_end) {
+                sv[q] = g.conj_t ? cconj(g.s[(long long)n * g.ld + m0 + lm]) : g.s[(long long)(m0 + lm) * g.ld + n];
+            } else {
+                sv[q] = make_double2(0.0, 0.0);
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { As[lm * kDT + lc + q] = av[q]; Ss[lm * (kDT + 1) + lc + q] = sv[q]; }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < kDK; ++kk) {
+            cd x[4], y[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) x[i] = Ss[kk * (kDT + 1) + ty + 16 * i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) y[j] = As[kk * kDT + tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {           // acc += x y
+                    acc[i][j].x = fma(x[i].x, y[j].x, fma(-x[i].y, y[j].y, acc[i][j].x));
+                    acc[i][j].y = fma(x[i].x, y[j].y, fma(x[i].y, y[j].x, acc[i][j].y));
+                }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int n = n0 + ty + 16 * i;
+            const long long r = r0 + tx + 16 * j;
+            if (n >= n_end || r >= g.n_pts) continue;
+            const long long k = (long long)n * g.n_pts + r;
+            cd v = acc[i][j];
+            if (g.mode == 1) {
+                v = csub(g.h[k], v);
+            } else if (g.mode == 2) {
+                const cd d = csub(g.h[k], v), pv = g.p[k], qv = g.q[k];
+                v = make_double2(pv.x + g.fx * d.x - g.fy * d.y - qv.x, pv.y + g.fx * d.y + g.fy * d.x - qv.y);
+            } else if (g.mode == 3) {
+                v = csub(g.out[k], v);
+            }
+            g.out[k] = v;
+        }
+}
+
+// ---- density: part[s][r] = sum over this split's orbitals of |psi_i(r)|^2; rho = sum_s part (fixed order) -----------------
+__global__ void __launch_bounds__(256) density_partial(const cd *psi, long long n_pts, int n, int per_split, double *part) {
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_pts) return;
+    const int i_beg = blockIdx.y * per_split, i_end = min(n, i_beg + per_split);
+    double s = 0.0;
+    for (int i = i_beg; i < i_end; ++i) {
+        const cd z = psi[(long long)i * n_pts + r];
+        s = fma(z.x, z.x, fma(z.y, z.y, s));
+    }
+    part[(long long)blockIdx.y * n_pts + r] = s;
+}
+__global__ void __launch_bounds__(256) density_reduce(const double *part, long long n_pts, int splits, double *rho) {
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_pts) return;
+    double s = part[r];
+    for (int q = 1; q < splits; ++q) s += part[(long long)q * n_pts + r];
+    rho[r] = s;
+}
+
+// ---- blocked Cholesky of S (np x np, np a multiple of 64, row major, lower triangle) -----------------------------------
+// panel k: chol_diag factors the 64 x 64 diagonal block in shared memory; tri_solve_block solves the rows below against
+// it (L21 = A21 L11^{-H}); chol_update subtracts L21 L21^H from the trailing lower triangle.
+constexpr int kBlkSmem = 64 * 65 * (int)sizeof(cd);       // one padded 64 x 64 block (dynamic shared memory)
+
+// diag0[k] = S[k][k] before the factorisation: the scale a pivot is judged against
+__global__ void __launch_bounds__(256) save_diag(const cd *s, int ld, int np, double *diag0) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < np) diag0[k] = s[(long long)k * ld + k].x;
+}
+
+// a pivot below 1e-12 of the column's original diagonal means a numerically dependent column: flagged in *info
+__global__ void __launch_bounds__(64) chol_diag(cd *s, int ld, int k0, const double *diag0, int *info) {
+    extern __shared__ __align__(16) unsigned char dense_smem[];
+    cd *L = reinterpret_cast<cd *>(dense_smem);
+    const int t = threadIdx.x;                            // row
+    for (int c = 0; c < 64; ++c) L[t * 65 + c] = s[(long long)(k0 + t) * ld + k0 + c];
+    __syncthreads();
+    for (int c = 0; c < 64; ++c) {
+        // column c: d = sqrt(L[c][c] - sum_{k<c} |L[c][k]|^2); rows t > c: (L[t][c] - sum_k L[t][k] conj(L[c][k])) / d
+        cd v = L[t * 65 + c];
+        for (int k = 0; k < c; ++k) {
+            const cd x = L[t * 65 + k], y = L[c * 65 + k];
+            v.x -= x.x * y.x + x.y * y.y;
+            v.y -= x.y * y.x - x.x * y.y;
+        }
+        __syncthreads();
+        if (t == c) {
+            if (!(v.x > 1e-12 * diag0[k0 + c])) { atomicCAS(info, 0, k0 + c + 1); v.x = 1.0; }
+            L[c * 65 + c] = make_double2(sqrt(v.x), 0.0);
+        }
+        __syncthreads();
+        if (t > c) {
+            const double d = 1.0 / L[c * 65 + c].x;
+            L[t * 65 + c] = make_double2(v.x * d, v.y * d);
+        } else if (t < c) {
+            L[t * 65 + c] = make_double2(0.0, 0.0);
+        }
+        __syncthreads();
+    }
+    for (int c = 0; c < 64; ++c) s[(long long)(k0 + t) * ld + k0 + c] = L[t * 65 + c];
+}
+
+// trailing update: tile (bi >= bj) of A22 -= L21(bi) L21(bj)^H, K = 64.  grid.x = lower-triangular tile index.
+__global__ void __launch_bounds__(256) chol_update(cd *s, int ld, int k0, int np) {
+    __shared__ cd Ri[kDT * kDP], Rj[kDT * kDP];
+    int bi = 0, idx = blockIdx.x;
+    while (idx > bi) { idx -= bi + 1; ++bi; }             // blockIdx.x = bi (bi + 1) / 2 + bj
+    const int bj = idx;
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int i0 = k0 + 64 + bi * 64, j0 = k0 + 64 + bj * 64;
+    const int lrow = tid >> 2, lk = (tid & 3) * 4;
+    cd acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
+    for (int kc = 0; kc < 64; kc += kDK) {
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            Ri[lrow * kDP + lk + q] = s[(long long)(i0 + lrow) * ld + k0 + kc + lk + q];
+            Rj[lrow * kDP + lk + q] = s[(long long)(j0 + lrow) * ld + k0 + kc + lk + q];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < kDK; ++kk) {
+            cd x[4], y[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) x[i] = Ri[(ty + 16 * i) * kDP + kk];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) y[j] = Rj[(tx + 16 * j) * kDP + kk];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {           // acc += x conj(y)
+                    acc[i][j].x = fma(x[i].x, y[j].x, fma(x[i].y, y[j].y, acc[i][j].x));
+                    acc[i][j].y = fma(x[i].y, y[j].x, fma(-x[i].x, y[j].y, acc[i][j].y));
+                }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int r = i0 + ty + 16 * i, c = j0 + tx + 16 * j;
+            if (c > r) continue;
+            cd *p = s + (long long)r * ld + c;
+            *p = csub(*p, acc[i][j]);
+        }
+}
+
+// identity on the padding (rows / columns n .. np - 1) so that the padded matrix factors as blockdiag(L, I)
+__global__ void __launch_bounds__(256) pad_identity(cd *s, int ld, int n, int np) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= (long long)np * np) return;
+    const int r = (int)(k / np), c = (int)(k % np);
+    if (r >= n || c >= n) s[(long long)r * ld + c] = make_double2(r == c ? 1.0 : 0.0, 0.0);
+}
+
+// ---- triangular solve against one 64 x 64 diagonal block: X L^H = Y in place, one thread per vector --------------------
+// vector v, column c lives at x[v * v_stride + c * c_stride]: orbitals (v = grid point: v_stride 1, c_stride n_pts) for
+// Psi <- Psi L^{-H} ("Trsm"), rows of S (v = row: v_stride ld, c_stride 1) for the Cholesky panel
+// L21 = A21 L11^{-H}.  16 columns at a time in registers: x_c = (y_c - sum_{k<c} x_k conj(L[c][k])) / L[c][c].
+__global__ void __launch_bounds__(128) tri_solve_block(cd *x, long long n_vec, long long v_stride, long long c_stride,
+                                                       const cd *l, int ld, int c0, int nc) {
+    extern __shared__ __align__(16) unsigned char dense_smem[];
+    cd *L = reinterpret_cast<cd *>(dense_smem);
+    for (int e = threadIdx.x; e < 64 * 64; e += blockDim.x) {
+        const int rr = e >> 6, c = e & 63;
+        L[rr * 65 + c] = (rr < nc && c < nc) ? l[(long long)(c0 + rr) * ld + c0 + c] : make_double2(rr == c ? 1.0 : 0.0, 0.0);
+    }
+    __syncthreads();
+    const long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= n_vec) return;
+    cd *xv = x + v * v_stride;
+    for (int sb = 0; sb < nc; sb += 16) {
+        cd t[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) t[c] = (sb + c < nc) ? xv[(long long)(sb + c) * c_stride] : make_double2(0.0, 0.0);
+        for (int m = 0; m < sb; ++m) {                    // this block's finished columns (read back: final values)
+            const cd xm = xv[(long long)m * c_stride];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const cd y = L[(sb + c) * 65 + m];
+                t[c].x -= xm.x * y.x + xm.y * y.y;
+                t[c].y -= xm.y * y.x - xm.x * y.y;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            cd u = t[c];
+#pragma unroll
+            for (int k = 0; k < c; ++k) {
+                const cd y = L[(sb + c) * 65 + sb + k];
+                u.x -= t[k].x * y.x + t[k].y * y.y;
+                u.y -= t[k].y * y.x - t[k].x * y.y;
+            }
+            const double d = 1.0 / L[(sb + c) * 65 + sb + c].x;
+            t[c] = make_double2(u.x * d, u.y * d);
+        }
+#pragma unroll
+        for (int c = 0; c < 16; ++c)
+            if (sb + c < nc) xv[(long long)(sb + c) * c_stride] = t[c];
+    }
+}
+
+}  // namespace ptfock

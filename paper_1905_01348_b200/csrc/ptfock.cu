@@ -7,12 +7,14 @@
 #include "pencil_tma.cuh"
 #include "pass8.cuh"
 #include "onchip16.cuh"
+#include "dense.cuh"
 
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <initializer_list>
 #include <new>
 #include <vector>
 
@@ -212,6 +214,8 @@ struct ptfock_plan {
     std::vector<cudaEvent_t> *copy_ev;
     int sm_count;
     cd *ones;                           // ptfock_debug_pair: a grid of ones (lazily allocated)
+    int *chol_info;                     // ptfock_orthonormalize: first non-positive pivot (device), and its pinned host copy
+    int *chol_info_host;
     // cross-stream ordering: the plan's scratch is shared by consecutive calls, so a call on another stream first
     // waits for the event the previous call recorded at its end
     cudaEvent_t busy_ev;
@@ -259,6 +263,8 @@ void free_plan(ptfock_plan *p) {
     cudaFree(p->st_psi);
     cudaFree(p->st_out);
     cudaFree(p->ones);
+    cudaFree(p->chol_info);
+    if (p->chol_info_host) cudaFreeHost(p->chol_info_host);
     if (p->busy_ev) cudaEventDestroy(p->busy_ev);
     if (p->ev_pool) { for (cudaEvent_t e : *p->ev_pool) cudaEventDestroy(e); delete p->ev_pool; }
     if (p->copy_ev) { for (cudaEvent_t e : *p->copy_ev) cudaEventDestroy(e); delete p->copy_ev; }
@@ -474,9 +480,18 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     while ((size_t)Ib * Jb * pair_bytes > limit && Ib > 1) Ib = (Ib + 1) / 2;
     while ((size_t)Ib * Jb * pair_bytes > limit && Jb > 1) Jb = (Jb + 1) / 2;
     if ((size_t)Ib * Jb * pair_bytes > limit) { free_plan(p); return PTFOCK_ERR_ALLOC; }
+    // the dense-algebra calls keep an n x n matrix (padded to the 64-wide blocks) and a few split-K partial sums in the
+    // same scratch: never size it below that
+    size_t dense_min = 0;
+    {
+        const size_t nmax = (size_t)std::max(d.n_occ, d.max_targets), npad = (nmax + 63) / 64 * 64;
+        const size_t tiles = (npad / 64) * (npad / 64);
+        const size_t ks = std::max<size_t>(1, std::min<size_t>(8, (4 * (size_t)prop.multiProcessorCount + tiles - 1) / tiles));
+        dense_min = sizeof(cd) * (npad * npad + npad + ks * nmax * nmax);
+    }
     // a failing allocation (fragmentation, another allocator holding the memory) shrinks the wave instead of failing
     for (;;) {
-        p->scratch_bytes = (size_t)Ib * Jb * pair_bytes;
+        p->scratch_bytes = std::max((size_t)Ib * Jb * pair_bytes, dense_min);
         cudaError_t e = cudaMalloc(&p->scratch, p->scratch_bytes);
         if (e == cudaSuccess) break;
         cudaGetLastError();
@@ -548,6 +563,7 @@ extern "C" const char *ptfock_strerror(int code) {
         case PTFOCK_ERR_ALLOC: return "allocation failed or workspace too small";
         case PTFOCK_ERR_CUDA: return "CUDA runtime error (see ptfock_last_cuda_error)";
         case PTFOCK_ERR_ALIAS: return "out overlaps an input";
+        case PTFOCK_ERR_NOT_POSITIVE: return "overlap matrix is not positive definite (linearly dependent orbitals)";
         default: return "unknown error";
     }
 }
@@ -952,6 +968,184 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
     if (w.err != cudaSuccess) { g_last_cuda = (int)w.err; return PTFOCK_ERR_CUDA; }
     CU(end_call(plan, st));
     return PTFOCK_OK;
+}
+
+// ================================================================================================
+// dense-algebra neighbours (dense.cuh): PAPER.md Alg. 3 (Sec. 3.3), Sec. 3.4
+// ================================================================================================
+namespace {
+
+int check_dev_ptrs(const ptfock_plan *p, std::initializer_list<const void *> ptrs) {
+    for (const void *q : ptrs) {
+        if (!q) continue;
+        if ((uintptr_t)q & 15) return PTFOCK_ERR_ALIGNMENT;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, q) != cudaSuccess) { cudaGetLastError(); return PTFOCK_ERR_INVALID_ARG; }
+        if (at.type == cudaMemoryTypeManaged) continue;
+        if (at.type != cudaMemoryTypeDevice || at.device != p->d.device) return PTFOCK_ERR_INVALID_ARG;
+    }
+    return PTFOCK_OK;
+}
+
+// S (n_a x n_b, row pitch ld_s) = w * A^H B; split-K partial sums go to `work` (bytes available: work_bytes)
+int overlap_into(ptfock_plan *p, const cd *a, int n_a, const cd *b, int n_b, cd *s, int ld_s, cd *work, size_t work_bytes,
+                 cudaStream_t st) {
+    const int tiles = ((n_a + kDT - 1) / kDT) * ((n_b + kDT - 1) / kDT);
+    long long ks = (4LL * p->sm_count + tiles - 1) / tiles;
+    ks = std::max(1LL, std::min(ks, p->N / 1024 > 0 ? p->N / 1024 : 1LL));
+    const size_t per = sizeof(cd) * (size_t)n_a * n_b;
+    ks = std::min<long long>(ks, (long long)(work_bytes / per));
+    if (ks < 1) return PTFOCK_ERR_ALLOC;
+    long long pps = (p->N + ks - 1) / ks;
+    pps = (pps + kDK - 1) / kDK * kDK;
+    ks = (p->N + pps - 1) / pps;
+    OverlapArgs g;
+    g.a = a; g.b = b; g.part = work; g.n_pts = p->N; g.pts_per_split = pps; g.n_a = n_a; g.n_b = n_b; g.ld = n_b;
+    overlap_partial<<<dim3((n_a + kDT - 1) / kDT, (n_b + kDT - 1) / kDT, (unsigned)ks), 256, 0, st>>>(g);
+    const long long cnt = (long long)n_a * n_b;
+    overlap_reduce<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(work, (int)ks, n_a, n_b, n_b, p->volume / (double)p->N, s, ld_s);
+    p->total_launches += 2;
+    return PTFOCK_OK;
+}
+
+void rotate_launch(ptfock_plan *p, const RotateArgs &g, cudaStream_t st) {
+    rotate_kernel<<<dim3((unsigned)((g.n_pts + kDT - 1) / kDT), (g.n_out + kDT - 1) / kDT), 256, 0, st>>>(g);
+    p->total_launches += 1;
+}
+
+}  // namespace
+
+extern "C" int ptfock_overlap(ptfock_plan *plan, const void *a, int32_t n_a, const void *b, int32_t n_b, void *s, void *stream) {
+    if (!plan || !a || !b || !s || n_a < 1 || n_b < 1) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { a, b, s });
+    if (rc != PTFOCK_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    rc = overlap_into(plan, (const cd *)a, n_a, (const cd *)b, n_b, (cd *)s, n_b, plan->scratch, plan->scratch_bytes, st);
+    if (rc != PTFOCK_OK) return rc;
+    CU(cudaGetLastError());
+    CU(end_call(plan, st));
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_rotate(ptfock_plan *plan, const void *a, int32_t n_a, const void *s, int32_t n_out, void *out, void *stream) {
+    if (!plan || !a || !s || !out || n_a < 1 || n_out < 1) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { a, s, out });
+    if (rc != PTFOCK_OK) return rc;
+    const size_t gbytes = sizeof(cd) * (size_t)plan->N;
+    if (overlaps(out, gbytes * n_out, a, gbytes * n_a)) return PTFOCK_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    RotateArgs g = {};
+    g.a = (const cd *)a; g.s = (const cd *)s; g.out = (cd *)out; g.n_pts = plan->N; g.n_a = n_a; g.n_out = n_out; g.ld = n_out;
+    rotate_launch(plan, g, st);
+    CU(cudaGetLastError());
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_residual(ptfock_plan *plan, const void *psi, const void *hpsi, const void *psi_half, int32_t n, double dt,
+                               void *r_out, void *stream) {
+    if (!plan || !psi || !hpsi || !r_out || n < 1 || !std::isfinite(dt)) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { psi, hpsi, psi_half, r_out });
+    if (rc != PTFOCK_OK) return rc;
+    const size_t gbytes = sizeof(cd) * (size_t)plan->N;
+    if (overlaps(r_out, gbytes * n, psi, gbytes * n)) return PTFOCK_ERR_ALIAS;      // every CTA reads all of Psi
+    const size_t s_bytes = sizeof(cd) * (size_t)n * n;
+    if (s_bytes * 2 > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    cd *S = plan->scratch;
+    rc = overlap_into(plan, (const cd *)psi, n, (const cd *)hpsi, n, S, n, plan->scratch + (size_t)n * n,
+                      plan->scratch_bytes - s_bytes, st);                          // Alg. 3 lines 2-3
+    if (rc != PTFOCK_OK) return rc;
+    RotateArgs g = {};
+    g.a = (const cd *)psi; g.s = S; g.h = (const cd *)hpsi; g.p = (const cd *)psi; g.q = (const cd *)psi_half; g.out = (cd *)r_out;
+    g.n_pts = plan->N; g.n_a = n; g.n_out = n; g.ld = n;
+    g.mode = psi_half ? 2 : 1;
+    g.fx = 0.0; g.fy = 0.5 * dt;                                                   // f = i dt / 2
+    rotate_launch(plan, g, st);                                                    // Alg. 3 lines 4-5 fused
+    CU(cudaGetLastError());
+    CU(end_call(plan, st));
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_density(ptfock_plan *plan, const void *psi, int32_t n, double *rho, void *stream) {
+    if (!plan || !psi || !rho || n < 1) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { psi });
+    if (rc != PTFOCK_OK) return rc;
+    if ((uintptr_t)rho & 7) return PTFOCK_ERR_ALIGNMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    const long long blocks = (plan->N + 255) / 256;
+    int splits = (int)std::max<long long>(1, std::min<long long>(n, (8LL * plan->sm_count + blocks - 1) / blocks));
+    splits = (int)std::min<size_t>((size_t)splits, plan->scratch_bytes / (sizeof(double) * (size_t)plan->N));
+    if (splits < 1) return PTFOCK_ERR_ALLOC;
+    const int per = (n + splits - 1) / splits;
+    splits = (n + per - 1) / per;
+    double *part = reinterpret_cast<double *>(plan->scratch);
+    density_partial<<<dim3((unsigned)blocks, splits), 256, 0, st>>>((const cd *)psi, plan->N, n, per, part);
+    density_reduce<<<(unsigned)blocks, 256, 0, st>>>(part, plan->N, splits, rho);
+    plan->total_launches += 2;
+    CU(cudaGetLastError());
+    CU(end_call(plan, st));
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, void *stream) {
+    if (!plan || !psi || n < 1) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { psi });
+    if (rc != PTFOCK_OK) return rc;
+    const int np = (n + 63) / 64 * 64;
+    const size_t s_bytes = sizeof(cd) * ((size_t)np * np + np);        // S, then the saved diagonal
+    if (s_bytes + sizeof(cd) * (size_t)n * n > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    if (!plan->chol_info) {
+        CU(cudaFuncSetAttribute(chol_diag, cudaFuncAttributeMaxDynamicSharedMemorySize, kBlkSmem));
+        CU(cudaFuncSetAttribute(tri_solve_block, cudaFuncAttributeMaxDynamicSharedMemorySize, kBlkSmem));
+        if (cudaMalloc(&plan->chol_info, sizeof(int)) != cudaSuccess) return PTFOCK_ERR_ALLOC;
+        if (cudaMallocHost(&plan->chol_info_host, sizeof(int)) != cudaSuccess) return PTFOCK_ERR_ALLOC;
+    }
+    CU(begin_call(plan, st));
+    cd *S = plan->scratch, *X = (cd *)psi;
+    CU(cudaMemsetAsync(plan->chol_info, 0, sizeof(int), st));
+    // S = Psi^* Psi, padded with the identity to a multiple of the block size
+    double *diag0 = reinterpret_cast<double *>(plan->scratch + (size_t)np * np);
+    rc = overlap_into(plan, X, n, X, n, S, np, plan->scratch + (size_t)np * np + np, plan->scratch_bytes - s_bytes, st);
+    if (rc != PTFOCK_OK) return rc;
+    if (np != n) pad_identity<<<(unsigned)(((long long)np * np + 255) / 256), 256, 0, st>>>(S, np, n, np);
+    save_diag<<<(np + 255) / 256, 256, 0, st>>>(S, np, np, diag0);
+    // blocked right-looking Cholesky S = L L^H (lower triangle, in place)
+    for (int k0 = 0; k0 < np; k0 += 64) {
+        chol_diag<<<1, 64, kBlkSmem, st>>>(S, np, k0, diag0, plan->chol_info);
+        const int below = np - k0 - 64;
+        if (below > 0) {
+            tri_solve_block<<<(below + 127) / 128, 128, kBlkSmem, st>>>(S + (size_t)(k0 + 64) * np + k0, below, np, 1, S, np, k0, 64);
+            const int t = below / 64;
+            chol_update<<<t * (t + 1) / 2, 256, 0, st>>>(S, np, k0, np);
+            plan->total_launches += 2;
+        }
+        plan->total_launches += 1;
+    }
+    // Psi <- Psi L^{-H}, 64 columns at a time: subtract the finished columns' part, then solve against the diagonal block
+    for (int c0 = 0; c0 < n; c0 += 64) {
+        const int nc = std::min(64, n - c0);
+        if (c0 > 0) {
+            RotateArgs g = {};
+            g.a = X; g.s = S; g.out = X; g.n_pts = plan->N; g.n_a = c0; g.n_out = nc; g.ld = np; g.conj_t = 1; g.mode = 3; g.n_first = c0;
+            rotate_launch(plan, g, st);
+        }
+        tri_solve_block<<<(unsigned)((plan->N + 127) / 128), 128, kBlkSmem, st>>>(X + (size_t)c0 * plan->N, plan->N, 1, plan->N, S, np, c0, nc);
+        plan->total_launches += 1;
+    }
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(plan->chol_info_host, plan->chol_info, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(end_call(plan, st));
+    CU(cudaStreamSynchronize(st));
+    return *plan->chol_info_host ? PTFOCK_ERR_NOT_POSITIVE : PTFOCK_OK;
 }
 
 extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
