@@ -46,7 +46,8 @@ typedef struct ptfock_plan ptfock_plan; /* opaque, owned by the library */
 
 enum {
     PTFOCK_KERNEL_COULOMB = 0,
-    PTFOCK_KERNEL_HSE = 1
+    PTFOCK_KERNEL_HSE = 1,
+    PTFOCK_KERNEL_KINETIC = 2           /* not an interaction: |G|^2 / 2, for ptfock_hloc_apply's plan (n_occ must be 1) */
 };
 
 enum {
@@ -145,6 +146,27 @@ int ptfock_density(ptfock_plan *plan, const void *psi, int32_t n, double *rho, v
  * (psi_m, psi_n) = delta_mn.  Synchronises `stream`; PTFOCK_ERR_NOT_POSITIVE if a pivot is not positive (psi is then
  * left modified). */
 int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, void *stream);
+
+/* ---- pieces of one PT-CN time step with a MODEL Hamiltonian (Alg. 1) -----------
+ * H[Psi] psi = -1/2 Laplacian psi + v_loc psi + V_X[Psi] psi: a real Hamiltonian needs the pseudopotentials the paper
+ * uses, which are not available; the model keeps the structure of Alg. 1 (residuals, fixed point with
+ * Anderson mixing over per-wavefunction least squares PAPER.md:194-198, density, re-orthogonalisation).  The step itself
+ * is sequenced by paper_1905_01348_b200/ptcn.py; every operation on grids goes through the calls of this header. */
+
+/* out_j = -1/2 Laplacian psi_j + vloc psi_j, j < n, on a plan created with kernel = PTFOCK_KERNEL_KINETIC, n_occ = 1
+ * (the kinetic operator runs through the same three passes as the exchange operator: a pair-solve with the constant
+ * orbital and the table |G|^2 / 2).  vloc: N doubles (DEVICE) or NULL.  out must not overlap psi.  Asynchronous. */
+int ptfock_hloc_apply(ptfock_plan *plan, const double *vloc, const void *psi, int32_t n, void *out, void *stream);
+
+/* out_j = a_j x_j + b_j y_j, j < n, with per-orbital complex coefficients from HOST arrays of n (re, im) pairs (the mixing
+ * coefficients of PAPER.md:194 are per wavefunction); y and b_host may be NULL.  out may be x or y.  Asynchronous; the
+ * host arrays may be reused when the call returns. */
+int ptfock_axpby(ptfock_plan *plan, int32_t n, const double *a_host, const void *x, const double *b_host, const void *y,
+                 void *out, void *stream);
+
+/* out_host[j] = (a_j, b_j) = (Omega/N) sum_r conj(a_j(r)) b_j(r), j < n (n (re, im) pairs, HOST): the entries of the
+ * per-wavefunction least-squares problems of the Anderson mixing.  Synchronises `stream`. */
+int ptfock_banddot(ptfock_plan *plan, const void *a, const void *b, int32_t n, double *out_host, void *stream);
 
 /* Frees everything the plan owns.  NULL is allowed. */
 int ptfock_destroy(ptfock_plan *plan);

@@ -17,12 +17,14 @@ SRC_DIR = os.path.join(_HERE, "csrc")
 
 KERNEL_COULOMB = 0
 KERNEL_HSE = 1
+KERNEL_KINETIC = 2
 FLAG_THREE_STAGE_SLABS = 1
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
            "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_copy_bandwidth",
-           "ptfock_overlap", "ptfock_rotate", "ptfock_residual", "ptfock_density", "ptfock_orthonormalize"]
+           "ptfock_overlap", "ptfock_rotate", "ptfock_residual", "ptfock_density", "ptfock_orthonormalize",
+           "ptfock_hloc_apply", "ptfock_axpby", "ptfock_banddot"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "1886"]
@@ -85,6 +87,9 @@ def lib() -> ctypes.CDLL:
         L.ptfock_residual.argtypes = [vp, vp, vp, vp, i32, ctypes.c_double, vp, vp]
         L.ptfock_density.argtypes = [vp, vp, i32, vp, vp]
         L.ptfock_orthonormalize.argtypes = [vp, vp, i32, vp]
+        L.ptfock_hloc_apply.argtypes = [vp, vp, vp, i32, vp, vp]
+        L.ptfock_axpby.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+        L.ptfock_banddot.argtypes = [vp, vp, vp, i32, vp, vp]
         for name in EXPORTS:
             if name != "ptfock_strerror":
                 getattr(L, name).restype = ctypes.c_int
@@ -265,6 +270,45 @@ class Plan:
         _check(lib().ptfock_orthonormalize(self._h, _dev_ptr(psi, "psi", self.device), n, _stream(self.device)),
                "ptfock_orthonormalize")
         return psi
+
+    # ---- PT-CN step helpers (Alg. 1) -------------------------------------------------------------------
+    def hloc_apply(self, psi, vloc=None, out=None):
+        """out_j = -1/2 Laplacian psi_j + vloc psi_j (plan created with KERNEL_KINETIC, n_occ = 1)."""
+        import torch
+        n = self._grids(psi, "psi")
+        if out is None:
+            out = torch.empty_like(psi)
+        vp_ = ctypes.c_void_p(0)
+        if vloc is not None:
+            if not (vloc.is_cuda and vloc.dtype == torch.float64 and vloc.is_contiguous() and vloc.numel() == self.N):
+                raise TypeError("vloc must be a contiguous float64 CUDA tensor of one grid")
+            vp_ = ctypes.c_void_p(vloc.data_ptr())
+        _check(lib().ptfock_hloc_apply(self._h, vp_, _dev_ptr(psi, "psi", self.device), n,
+                                       _dev_ptr(out, "out", self.device), _stream(self.device)), "ptfock_hloc_apply")
+        return out
+
+    def axpby(self, a, x, b=None, y=None, out=None):
+        """out_j = a_j x_j + b_j y_j; a, b: scalars or per-orbital sequences of complex numbers."""
+        import numpy as np
+        import torch
+        n = self._grids(x, "x")
+        av = np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=np.complex128), (n,)))
+        bv = None if y is None else np.ascontiguousarray(np.broadcast_to(np.asarray(b, dtype=np.complex128), (n,)))
+        if out is None:
+            out = torch.empty_like(x)
+        _check(lib().ptfock_axpby(self._h, n, ctypes.c_void_p(av.ctypes.data), _dev_ptr(x, "x", self.device),
+                                  ctypes.c_void_p(0 if bv is None else bv.ctypes.data), _dev_ptr(y, "y", self.device),
+                                  _dev_ptr(out, "out", self.device), _stream(self.device)), "ptfock_axpby")
+        return out
+
+    def banddot(self, a, b):
+        """numpy array of (a_j, b_j), j < n."""
+        import numpy as np
+        n = self._grids(a, "a")
+        res = np.empty(n, dtype=np.complex128)
+        _check(lib().ptfock_banddot(self._h, _dev_ptr(a, "a", self.device), _dev_ptr(b, "b", self.device), n,
+                                    ctypes.c_void_p(res.ctypes.data), _stream(self.device)), "ptfock_banddot")
+        return res
 
     def info(self) -> dict:
         a = (ctypes.c_int64 * 8)()

@@ -304,6 +304,8 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, b
                 double val;
                 if ((m0 | m1 | m2) == 0)
                     val = (d.kernel == PTFOCK_KERNEL_HSE) ? 0.5 * two_pi / (d.omega * d.omega) : 0.0;
+                else if (d.kernel == PTFOCK_KERNEL_KINETIC)
+                    val = 0.5 * g2;
                 else if (d.kernel == PTFOCK_KERNEL_HSE)
                     val = four_pi / g2 * (-std::expm1(-g2 * inv4w2));
                 else
@@ -320,7 +322,8 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, b
                 const double y = vnat[((size_t)((n0 - k0) % n0) * n1 + (n1 - k1) % n1) * n2 + (n2 - k2) % n2];
                 if (std::fabs(x - y) > 1e-14 * (std::fabs(x) + std::fabs(y))) { even = false; break; }
             }
-    const double scale = -d.alpha / (double)N;
+    // exchange kernels: -alpha/N folded in; the kinetic 'kernel' of the model Hamiltonian (ptfock_hloc_apply): +1/N
+    const double scale = (d.kernel == PTFOCK_KERNEL_KINETIC ? 1.0 : -d.alpha) / (double)N;
     vperm.resize((size_t)N);
     if (onchip) {
         // onchip16.cuh: natural frequency order, stored [k2][k0][k1]
@@ -375,7 +378,9 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     if (!desc || !out) return PTFOCK_ERR_INVALID_ARG;
     const ptfock_desc &d = *desc;
     if (d.n_occ < 1 || d.max_targets < 1 || d.block_i < 0 || d.block_j < 0) return PTFOCK_ERR_INVALID_ARG;
-    if (d.kernel != PTFOCK_KERNEL_COULOMB && d.kernel != PTFOCK_KERNEL_HSE) return PTFOCK_ERR_INVALID_ARG;
+    if (d.kernel != PTFOCK_KERNEL_COULOMB && d.kernel != PTFOCK_KERNEL_HSE && d.kernel != PTFOCK_KERNEL_KINETIC)
+        return PTFOCK_ERR_INVALID_ARG;
+    if (d.kernel == PTFOCK_KERNEL_KINETIC && d.n_occ != 1) return PTFOCK_ERR_INVALID_ARG;   // its one "orbital" is the constant 1
     if (d.kernel == PTFOCK_KERNEL_HSE && !(d.omega > 0.0)) return PTFOCK_ERR_INVALID_ARG;
     if (!std::isfinite(d.alpha)) return PTFOCK_ERR_INVALID_ARG;
     for (int k = 0; k < 3; ++k) if (!edge_ok(d.n[k])) return PTFOCK_ERR_UNSUPPORTED_GRID;
@@ -1146,6 +1151,125 @@ extern "C" int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, vo
     CU(end_call(plan, st));
     CU(cudaStreamSynchronize(st));
     return *plan->chol_info_host ? PTFOCK_ERR_NOT_POSITIVE : PTFOCK_OK;
+}
+
+// ================================================================================================
+// PT-CN step helpers (Alg. 1, PAPER.md:194-198 Anderson mixing)
+// ================================================================================================
+namespace {
+__global__ void __launch_bounds__(256) add_vloc_kernel(const double *vloc, const cd *psi, cd *out, long long n_pts, long long total) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= total) return;
+    const double v = vloc[k % n_pts];
+    const cd z = psi[k];
+    cd o = out[k];
+    o.x = fma(v, z.x, o.x);
+    o.y = fma(v, z.y, o.y);
+    out[k] = o;
+}
+// out_j = a_j x_j + b_j y_j (y may be null)
+__global__ void __launch_bounds__(256) axpby_kernel(const cd *coef, int n, const cd *x, const cd *y, cd *out, long long n_pts) {
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (r >= n_pts) return;
+    const long long k = (long long)j * n_pts + r;
+    cd v = cmul(coef[j], x[k]);
+    if (y) v = cadd(v, cmul(coef[n + j], y[k]));
+    out[k] = v;
+}
+// part[j][b] = sum over block b's points of conj(a_j) b_j; out[j] = w * sum_b part[j][b] (fixed order)
+__global__ void __launch_bounds__(256) banddot_partial(const cd *a, const cd *b, long long n_pts, int blocks_per, double2 *part) {
+    __shared__ double2 red[256];
+    const int j = blockIdx.y;
+    double sr = 0.0, si = 0.0;
+    for (long long r = (long long)blockIdx.x * 256 + threadIdx.x; r < n_pts; r += (long long)blocks_per * 256) {
+        const cd x = a[(long long)j * n_pts + r], y = b[(long long)j * n_pts + r];
+        sr += x.x * y.x + x.y * y.y;
+        si += x.x * y.y - x.y * y.x;
+    }
+    red[threadIdx.x] = make_double2(sr, si);
+    __syncthreads();
+    for (int h = 128; h > 0; h >>= 1) {
+        if (threadIdx.x < h) { red[threadIdx.x].x += red[threadIdx.x + h].x; red[threadIdx.x].y += red[threadIdx.x + h].y; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[(long long)j * blocks_per + blockIdx.x] = red[0];
+}
+__global__ void __launch_bounds__(64) banddot_final(const double2 *part, int blocks_per, int n, double w, double2 *out) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    double sr = 0.0, si = 0.0;
+    for (int b = 0; b < blocks_per; ++b) { sr += part[(long long)j * blocks_per + b].x; si += part[(long long)j * blocks_per + b].y; }
+    out[j] = make_double2(sr * w, si * w);
+}
+}  // namespace
+
+extern "C" int ptfock_hloc_apply(ptfock_plan *plan, const double *vloc, const void *psi, int32_t n, void *out, void *stream) {
+    if (!plan || !psi || !out || n < 1 || plan->d.kernel != PTFOCK_KERNEL_KINETIC) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { psi, out });
+    if (rc != PTFOCK_OK) return rc;
+    if (vloc && ((uintptr_t)vloc & 7)) return PTFOCK_ERR_ALIGNMENT;
+    const size_t gbytes = sizeof(cd) * (size_t)plan->N;
+    if (overlaps(out, gbytes * n, psi, gbytes * n)) return PTFOCK_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    if (!plan->ones) {
+        cudaError_t e = cudaMalloc(&plan->ones, gbytes);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
+        fill_ones<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(plan->ones, plan->N);
+    }
+    // T psi_j = IFFT[ |G|^2/2 FFT(conj(1) psi_j) ] * 1: the exchange passes with the constant orbital and the kinetic table
+    rc = apply_device(plan, plan->ones, (const cd *)psi, 0, n, (cd *)out, st);
+    if (rc != PTFOCK_OK) return rc;
+    if (vloc) {
+        const long long total = plan->N * (long long)n;
+        add_vloc_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(vloc, (const cd *)psi, (cd *)out, plan->N, total);
+        plan->total_launches += 1;
+    }
+    CU(cudaGetLastError());
+    CU(end_call(plan, st));
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_axpby(ptfock_plan *plan, int32_t n, const double *a_host, const void *x, const double *b_host, const void *y,
+                            void *out, void *stream) {
+    if (!plan || !a_host || !x || !out || n < 1 || (y && !b_host)) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { x, y, out });
+    if (rc != PTFOCK_OK) return rc;
+    if (sizeof(cd) * 2 * (size_t)n > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    // the coefficients travel through the head of the scratch (pageable host memory: the copy is staged by the runtime
+    // before the call returns, so the caller may reuse a_host / b_host at once)
+    CU(cudaMemcpyAsync(plan->scratch, a_host, sizeof(cd) * n, cudaMemcpyHostToDevice, st));
+    if (y) CU(cudaMemcpyAsync(plan->scratch + n, b_host, sizeof(cd) * n, cudaMemcpyHostToDevice, st));
+    axpby_kernel<<<dim3((unsigned)((plan->N + 255) / 256), n), 256, 0, st>>>(plan->scratch, n, (const cd *)x, (const cd *)y, (cd *)out, plan->N);
+    plan->total_launches += 1;
+    CU(cudaGetLastError());
+    CU(end_call(plan, st));
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_banddot(ptfock_plan *plan, const void *a, const void *b, int32_t n, double *out_host, void *stream) {
+    if (!plan || !a || !b || !out_host || n < 1) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { a, b });
+    if (rc != PTFOCK_OK) return rc;
+    const int blocks_per = (int)std::max<long long>(1, std::min<long long>(64, plan->N / 2048));
+    if (sizeof(double2) * (size_t)n * (blocks_per + 1) > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    CU(begin_call(plan, st));
+    double2 *part = reinterpret_cast<double2 *>(plan->scratch), *res = part + (size_t)n * blocks_per;
+    banddot_partial<<<dim3(blocks_per, n), 256, 0, st>>>((const cd *)a, (const cd *)b, plan->N, blocks_per, part);
+    banddot_final<<<(n + 63) / 64, 64, 0, st>>>(part, blocks_per, n, plan->volume / (double)plan->N, res);
+    plan->total_launches += 2;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out_host, res, sizeof(double2) * n, cudaMemcpyDeviceToHost, st));
+    CU(end_call(plan, st));
+    CU(cudaStreamSynchronize(st));
+    return PTFOCK_OK;
 }
 
 extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
