@@ -104,6 +104,51 @@ def test_replicas_only_bookkeeping_gloo_world2():
         assert mx == 4.0 and thr == pytest.approx(2 * 1000.0 / 4.0)
 
 
+def _gather_worker(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_1905_01348_b200 import harness
+    n_total, shape = 5, (2, 3, 2)
+    g = torch.Generator().manual_seed(7)
+    full = torch.complex(torch.randn((n_total,) + shape, generator=g, dtype=torch.float64),
+                         torch.randn((n_total,) + shape, generator=g, dtype=torch.float64))
+    lo, hi = harness.shard_range(n_total, world, rank)
+    got64 = harness.allgather_orbitals(full[lo:hi].clone(), n_total)
+    got32 = harness.allgather_orbitals(full[lo:hi].clone(), n_total, wire="fp32")
+    q.put((rank, (lo, hi), bool(torch.equal(got64, full)), float((got32 - full).abs().max() / full.abs().max())))
+    dist.destroy_process_group()
+
+
+def test_j_sharding_allgather_gloo_world2():
+    """N > 1 with Phi distributed: uneven blocks (3 + 2 of 5 orbitals) all-gathered bit-exactly in fp64; the fp32 wire
+    format of PAPER.md:154 costs at most single-precision rounding."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_gather_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [r[1] for r in res] == [(0, 3), (3, 5)]
+    for _, _, exact, err32 in res:
+        assert exact and 0.0 < err32 < 2.0 ** -23
+
+
+def test_shard_range_partitions():
+    from paper_1905_01348_b200 import harness
+    for n, world in ((3072, 8), (5, 2), (7, 3), (2, 4)):
+        parts = [harness.shard_range(n, world, r) for r in range(world)]
+        assert parts[0][0] == 0 and parts[-1][1] == n
+        assert all(parts[k][1] == parts[k + 1][0] for k in range(world - 1))
+        sizes = [hi - lo for lo, hi in parts]
+        assert max(sizes) - min(sizes) <= 1
+
+
 def test_harness_single_process_identity():
     from paper_1905_01348_b200 import harness
     assert harness.max_over_ranks(3.5) == 3.5
