@@ -397,8 +397,9 @@ def main():
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the second headline config (one Si1536 j-block) that the default Si512 run also times")
     ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")
-    ap.add_argument("--leg", default="fock", choices=["fock", "dense"],
-                    help="fock: the headline exchange path (default); dense: the dense-algebra neighbours, own JSON line")
+    ap.add_argument("--leg", default="fock", choices=["fock", "dense", "copybw"],
+                    help="fock: the headline exchange path (default); dense: the dense-algebra neighbours; copybw: device "
+                         "copy bandwidth vs working-set size (L2-resident vs HBM; profiles/r02_l2_resident.md); own JSON lines")
     args = ap.parse_args()
 
     from paper_1905_01348_b200 import synth
@@ -423,6 +424,16 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     binding.lib()                                   # fails loudly if the CUDA library is missing
+    if args.leg == "copybw":
+        if rank == 0:
+            res = {f"{mb} MiB": binding.measure_copy_bandwidth(mb << 20, reps=max(4, 2048 // mb), device=local)
+                   for mb in (16, 24, 32, 48, 64, 128, 512, 2048)}
+            print(json.dumps({"metric": "device-to-device copy, read + write GB/s vs source size (working set = 2x)",
+                              "unit": "GB/s", "l2_bytes": torch.cuda.get_device_properties(local).L2_cache_size,
+                              "copy_GBs": res}), flush=True)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     if args.leg == "dense":
         if rank == 0:
             dense_leg(cfg, args, dev, local)

@@ -119,7 +119,16 @@ struct SlabArgs {
     int stride_loop;    // scratch pair index = loop_local * stride_loop + cta_local * stride_cta
     int stride_cta;
     int conj_w;         // pass C: use conj(W) (pair symmetry W_ji = conj(W_ij))
+    int tri;            // diagonal block of the pair-symmetric schedule: 1 = loop index <= CTA index only (pairs i <= j),
+                        // 2 = loop index > CTA index only (the conj(W) accumulate of the same block); 0 = whole range
 };
+
+// loop range [lo, hi) of a slab pass for CTA index `cta` out of [beg, end)
+PTF_DEV void tri_range(int tri, int cta, int beg, int end, int &lo, int &hi) {
+    lo = beg; hi = end;
+    if (tri == 1) hi = min(end, cta + 1);
+    else if (tri == 2) lo = max(beg, cta + 1);
+}
 
 // ---- pass A ---------------------------------------------------------------------------------------
 // grid = (number of targets in the wave, n0, chunks of the i loop); CTA (jj, x0, z) loops over its share of
@@ -140,7 +149,8 @@ __global__ void __launch_bounds__(kSlabThreads) slab_fwd(const SlabArgs g) {
 #pragma unroll
     for (int k = 0; k < S::PER_THREAD; ++k) pj[k] = psi[tid + k * kSlabThreads];
     const int per = (g.na + gridDim.z - 1) / gridDim.z;
-    const int ii_beg = blockIdx.z * per, ii_end = min(g.na, ii_beg + per);
+    int ii_beg, ii_end;
+    tri_range(g.tri, jj, blockIdx.z * per, min(g.na, blockIdx.z * per + per), ii_beg, ii_end);
     for (int ii = ii_beg; ii < ii_end; ++ii) {
         const cd *phi = g.a + (long long)(g.a0 + ii) * g.grid_pts + slab_off;
 #pragma unroll
@@ -179,7 +189,9 @@ __global__ void __launch_bounds__(kSlabThreads) slab_inv_acc(const SlabArgs g) {
     cd acc[S::PER_THREAD];
 #pragma unroll
     for (int k = 0; k < S::PER_THREAD; ++k) acc[k] = make_double2(0.0, 0.0);
-    for (int ss = 0; ss < g.na; ++ss) {
+    int ss_beg, ss_end;
+    tri_range(g.tri, tt, 0, g.na, ss_beg, ss_end);
+    for (int ss = ss_beg; ss < ss_end; ++ss) {
         const cd *src = g.scratch + ((long long)(ss * g.stride_loop + tt * g.stride_cta) * g.n0 + x0) * S::NPTS;
 #pragma unroll
         for (int k = 0; k < S::PER_THREAD; ++k) {
@@ -227,6 +239,7 @@ struct PencilArgs {
     const double *v;     // [N0 positions][slab_pts], digit-permuted, -alpha/N folded in
     const cd *tw0;
     int slab_pts;
+    int tri_nj;          // > 0: diagonal block of the symmetric schedule, pair = i*tri_nj + j exists only for i <= j
 };
 
 template <int N0>
@@ -235,6 +248,7 @@ __global__ void __launch_bounds__(PencilShape<N0>::NT, PencilShape<N0>::MINB) pe
     constexpr int R1 = S::R1, R2 = S::R2, CW = S::CW, NT = S::NT;
     const int tid = threadIdx.x;
     const long long sp = g.slab_pts;
+    if (g.tri_nj > 0 && (int)blockIdx.y / g.tri_nj > (int)blockIdx.y % g.tri_nj) return;
     cd *base = g.scratch + (long long)blockIdx.y * N0 * sp;
     if (R2 == 1) {
         // whole pencil in one thread's registers: no shared memory at all

@@ -174,7 +174,8 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     const int tid = threadIdx.x;
     const int jj = blockIdx.x, x0 = blockIdx.y / S::NQ, q = blockIdx.y % S::NQ;
     const int per = (g.na + gridDim.z - 1) / gridDim.z;
-    const int ii_beg = blockIdx.z * per, ii_end = min(g.na, ii_beg + per);
+    int ii_beg, ii_end;
+    tri_range(g.tri, jj, blockIdx.z * per, min(g.na, blockIdx.z * per + per), ii_beg, ii_end);
     const int n_it = ii_end - ii_beg;
     if (n_it <= 0) return;
     // stage-1 task (r, b2): the 4 x 4 points (a1, a2) at x1 = a1*B1 + b1, x2 = a2*B2 + b2
@@ -273,12 +274,15 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
     const int tid = threadIdx.x;
     const int tt = blockIdx.x, x0 = blockIdx.y / S::NQ, q = blockIdx.y % S::NQ;
-    const int n_it = g.na;
+    int it_lo, it_hi;
+    tri_range(g.tri, tt, 0, g.na, it_lo, it_hi);
+    const int n_it = it_hi - it_lo;
     if (n_it <= 0) return;
     const int b2 = tid % B2, r = tid / B2, b1 = q * RQ + r;
     const long long off1 = (long long)x0 * (N1 * N2) + b1 * N2 + b2;
     const long long pair_stride = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
-    const cd *src = g.scratch + (((long long)tt * g.stride_cta * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS;
+    const cd *src = g.scratch + (((long long)tt * g.stride_cta * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS
+                    + (long long)it_lo * pair_stride;
     if (tid == 0) {
 #pragma unroll
         for (int k = 0; k < NBUF; ++k) mbar_init(&bars[k], 1);
@@ -299,7 +303,7 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     cd acc[A1 * A2];
 #pragma unroll
     for (int k = 0; k < A1 * A2; ++k) acc[k] = make_double2(0.0, 0.0);
-    const cd *phi = g.a + (long long)g.a0 * g.grid_pts + off1;
+    const cd *phi = g.a + (long long)(g.a0 + it_lo) * g.grid_pts + off1;
     cd f[A1 * A2];
 #pragma unroll
     for (int a1 = 0; a1 < A1; ++a1)
@@ -377,6 +381,7 @@ struct P8MidArgs {
     const double2 *v;    // [tile group][16][64 threads]: the middle-stage thread's v' values (k0b = 2m, 2m + 1)
     const cd *tw0;       // exp(-2 pi i t / N0)
     int n_pairs;         // pairs in the wave
+    int tri_nj;          // > 0: diagonal block of the symmetric schedule, pair = i*tri_nj + j exists only for i <= j
 };
 
 PTF_DEV void tensor_g2s_2d_sw(void *dst_smem, const CUtensorMap *map, int c0, int c1, unsigned long long *bar) {
@@ -417,7 +422,8 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
         bulk_g2s(smem_b + GB * S::TILE_B, g.v + (long long)grp_pos * (S::V_BYTES / 16), S::V_BYTES, &bars[GB]);
 #pragma unroll
         for (int k = 0; k < GB; ++k)
-            if (blockIdx.y * GB + k < g.n_pairs) {
+            if (blockIdx.y * GB + k < g.n_pairs &&
+                !(g.tri_nj > 0 && (int)(blockIdx.y * GB + k) / g.tri_nj > (int)(blockIdx.y * GB + k) % g.tri_nj)) {
                 mbar_expect_tx(&bars[k], S::TILE_B);
                 tensor_g2s_2d_sw(smem_b + k * S::TILE_B, &map, grp_pos * (P * RQ * 2), (blockIdx.y * GB + k) * S::ROWS, &bars[k]);
             }
@@ -431,7 +437,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
     const int mr = tid % RQ, mp = (tid / RQ) % P, mq = (tid / (RQ * P)) % NQ, mk = tid / (RQ * P * NQ);
     const int rb = (mq * N0 + mk * 32) * 8, mc = mp * RQ + mr;
     __syncthreads();                                    // mbarrier inits visible; from here on the groups are independent
-    if (pair >= g.n_pairs) return;
+    if (pair >= g.n_pairs || (g.tri_nj > 0 && pair / g.tri_nj > pair % g.tri_nj)) return;
     auto group_sync = [&]() {                           // named barrier 1 + gi over the group's 64 threads
         if (gi == 0) asm volatile("bar.sync 1, %0;" ::"n"(S::NTB) : "memory");
         else if (gi == 1) asm volatile("bar.sync 2, %0;" ::"n"(S::NTB) : "memory");

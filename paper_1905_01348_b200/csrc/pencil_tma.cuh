@@ -36,6 +36,7 @@ struct PencilTmaArgs {
     const double *v;     // [N0 positions][slab_pts], digit-permuted, -alpha/N folded in
     const cd *tw0;
     int slab_pts;
+    int tri_nj;          // see PencilArgs
 };
 
 // grid = (ceil(slab_pts / CW), pairs); the tensor map views the scratch as [pairs*N0 rows][2*slab_pts doubles]
@@ -50,6 +51,7 @@ pencil_tma(const __grid_constant__ CUtensorMap map, const PencilTmaArgs g) {
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_pt + S::TILE_BYTES + N0 * 16);
     const int tid = threadIdx.x;
     const long long sp = g.slab_pts;
+    if (g.tri_nj > 0 && (int)blockIdx.y / g.tri_nj > (int)blockIdx.y % g.tri_nj) return;
     const int p0 = blockIdx.x * CW;
     const int row0 = blockIdx.y * N0;
     if (tid == 0) {

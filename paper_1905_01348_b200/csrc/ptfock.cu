@@ -632,14 +632,14 @@ void mark(Wave &w, int tag) {
 }
 
 // A + B for the block of pairs (i in [i0, i0+ni)) x (j in [j0, j0+nj)); pair index = ii * nj + jj.
-void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int j0, int nj) {
+void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int j0, int nj, int tri = 0) {
     ptfock_plan *p = w.p;
     SlabArgs a;
     a.a = phi; a.b = psi; a.scratch = p->scratch; a.out = nullptr;
     a.tw1 = p->tw_dev[1]; a.tw2 = p->tw_dev[2];
     a.grid_pts = p->N; a.n0 = p->d.n[0];
     a.a0 = i0; a.na = ni; a.b0 = j0;
-    a.stride_loop = nj; a.stride_cta = 1; a.conj_w = 0;
+    a.stride_loop = nj; a.stride_cta = 1; a.conj_w = 0; a.tri = tri;
     // split the i loop over blockIdx.z until the grid has a few CTAs per SM
     int z = 1;
     const long long base = (long long)p->d.n[0] * nj;
@@ -651,39 +651,39 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
         mark(w, 0);
         P8MidArgs b;
         b.v = p->v8_dev; b.tw0 = p->tw_dev[0];
-        b.n_pairs = ni * nj;
+        b.n_pairs = ni * nj; b.tri_nj = tri ? nj : 0;
         p->p8->mid(p->tmap8, b, ni * nj, w.st);
         mark(w, 1);
         w.launches += 2;
-        w.pairs += (long long)ni * nj;
+        w.pairs += tri ? (long long)nj * (nj + 1) / 2 : (long long)ni * nj;
         return;
     }
     p->slab->fwd(a, dim3(nj, p->d.n[0], z), w.st);
     mark(w, 0);
     if (p->use_tma) {
         PencilTmaArgs b;
-        b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
+        b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts; b.tri_nj = tri ? nj : 0;
         p->pencil->run_tma(p->tmap, b, ni * nj, w.st);
     } else {
         PencilArgs b;
-        b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts;
+        b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts; b.tri_nj = tri ? nj : 0;
         p->pencil->run(b, ni * nj, w.st);
     }
     mark(w, 1);
     w.launches += 2;
-    w.pairs += (long long)ni * nj;
+    w.pairs += tri ? (long long)nj * (nj + 1) / 2 : (long long)ni * nj;
 }
 
 // C: out[t0 + tt] += sum_ss orb[s0 + ss] * W(ss, tt)
 void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, int nt, int stride_loop, int stride_cta,
-                     int conj_w) {
+                     int conj_w, int tri = 0) {
     ptfock_plan *p = w.p;
     SlabArgs a;
     a.a = orb; a.b = nullptr; a.scratch = p->scratch; a.out = out;
     a.tw1 = p->tw_dev[1]; a.tw2 = p->tw_dev[2];
     a.grid_pts = p->N; a.n0 = p->d.n[0];
     a.a0 = s0; a.na = ns; a.b0 = t0;
-    a.stride_loop = stride_loop; a.stride_cta = stride_cta; a.conj_w = conj_w;
+    a.stride_loop = stride_loop; a.stride_cta = stride_cta; a.conj_w = conj_w; a.tri = tri;
     if (p->p8) p->p8->inv(a, dim3(nt, p->d.n[0] * p->p8->nq, 1), w.st);
     else p->slab->inv(a, dim3(nt, p->d.n[0], 1), w.st);
     mark(w, 2);
@@ -794,9 +794,12 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
             for (int i0 = 0; i0 <= j0; i0 += bs) {
                 const int ni = (n_occ - i0 < bs) ? n_occ - i0 : bs;
                 if (hp) { hp->need(st, i0, i0 + ni); hp->need(st, j0, j0 + nj); }
-                wave_forward_mid(w, phi, phi, i0, ni, j0, nj);
-                wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
-                if (i0 != j0) wave_accumulate(w, phi, j0, nj, out, i0, ni, 1, nj, 1);
+                // diagonal blocks (i0 == j0): only the pairs i <= j are solved; W_ij then serves out_j (loop i <= j) and,
+                // through conj, out_i (loop j > i)
+                const int tri = (i0 == j0) ? 1 : 0;
+                wave_forward_mid(w, phi, phi, i0, ni, j0, nj, tri);
+                wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0, tri);
+                if (nj > 1 || !tri) wave_accumulate(w, phi, j0, nj, out, i0, ni, 1, nj, 1, tri ? 2 : 0);
             }
         }
     } else {

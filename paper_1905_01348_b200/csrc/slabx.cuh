@@ -212,7 +212,8 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_fwd(const SlabArgs g) {
     const int x0 = blockIdx.y, jj = blockIdx.x;
     const long long slab_off = (long long)x0 * S::NPTS;
     const int per = (g.na + gridDim.z - 1) / gridDim.z;
-    const int ii_beg = blockIdx.z * per, ii_end = min(g.na, ii_beg + per);
+    int ii_beg, ii_end;
+    tri_range(g.tri, jj, blockIdx.z * per, min(g.na, blockIdx.z * per + per), ii_beg, ii_end);
     const int n_it = ii_end - ii_beg;
     if (n_it <= 0) return;
     const cd *phi0 = g.a + (long long)(g.a0 + ii_beg) * g.grid_pts + slab_off;      // slab of the first orbital
@@ -377,10 +378,12 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
     const int tid = threadIdx.x, lane = tid & 31;
     const int x0 = blockIdx.y, tt = blockIdx.x;
     const long long slab_off = (long long)x0 * S::NPTS;
-    const int n_it = g.na;
+    int it_lo, it_hi;
+    tri_range(g.tri, tt, 0, g.na, it_lo, it_hi);
+    const int n_it = it_hi - it_lo;
     if (n_it <= 0) return;
     const long long pair_stride = (long long)g.stride_loop * g.n0 * S::NPTS;
-    const cd *src0 = g.scratch + ((long long)(tt * g.stride_cta) * g.n0 + x0) * S::NPTS;
+    const cd *src0 = g.scratch + ((long long)(tt * g.stride_cta) * g.n0 + x0) * S::NPTS + (long long)it_lo * pair_stride;
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < NBUF; ++b) mbar_init(&bars[b], 1);
@@ -397,7 +400,7 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
     }
     const int cb = tid % S::CB1, b1 = tid / S::CB1;
     const int base1 = s1_base<S, CL>(tid);
-    const cd *phi0 = g.a + (long long)g.a0 * g.grid_pts + slab_off + b1 * N2 + cb;
+    const cd *phi0 = g.a + (long long)(g.a0 + it_lo) * g.grid_pts + slab_off + b1 * N2 + cb;
     const bool act1 = S::NT1 == NT || tid < S::NT1;      // this thread owns a last-stage task (and its accumulators)
     cd acc[R1 * C1];
 #pragma unroll
@@ -513,7 +516,7 @@ __global__ void __launch_bounds__(S::NT, S::MINB) slabx_inv_acc(const SlabArgs g
         cd *T = tiles + (it % NBUF) * TILE;
         const cd *phi = phi0 + (long long)it * g.grid_pts;
         if (tid == 0 && it + 1 < n_it)      // next orbital's slab into L2 while this one is transformed
-            l2_prefetch(g.a + (long long)(g.a0 + it + 1) * g.grid_pts + slab_off, S::NPTS * 16u);
+            l2_prefetch(g.a + (long long)(g.a0 + it_lo + it + 1) * g.grid_pts + slab_off, S::NPTS * 16u);
         // here: stage 1' of pair it and stage 3' of pair it-1 are done by this thread
         fence_proxy_async();
         __syncthreads();
