@@ -23,16 +23,6 @@
 #include "kernels.cuh"
 #include "tma.cuh"
 
-#ifndef P8_A_PREF
-#define P8_A_PREF 0          // 1: pass A prefetches the next phi_i through registers (255 registers, 4 CTAs per SM)
-#endif
-#ifndef P8_C_PREF
-#define P8_C_PREF 0          // 1: pass C prefetches the next pair density through registers (255 registers)
-#endif
-#ifndef P8_C_L2PF
-#define P8_C_L2PF 2          // pass C: L2 prefetch distance (iterations) for the pair-density rows, 0 = off
-#endif
-
 namespace ptfock {
 
 template <int N0_, int N1_, int N2_, int A1_, int A2_, int A0_>
@@ -46,8 +36,6 @@ struct P8 {
     static constexpr int NT = RQ * B2;                      // slab passes: stage-1 tasks (r, b2)
     static constexpr int NT2 = A1 * A2 * RQ;                // stage-2 tasks (k1a, k2a, r)
     static_assert(NT == NT2 && NT == 64, "one task per thread in both stages");
-    static constexpr int PW = B2 + 1;                       // exchange tile pitch (elements): conflict free both ways
-    static constexpr int WORK = NT2 * PW;
     static constexpr int QPTS = A1 * RQ * N2;               // points of one (slab, q) row of the scratch
     static constexpr int NPOS = A1 * A2 * B2;               // slab positions (k2b, k1a, k2a) per row
     static constexpr int NBUF_A = 2;                        // pass A: ring of landed phi_i quarter slabs
@@ -145,10 +133,6 @@ template <int R, int C, bool INV> PTF_DEV void dft_cols(cd (&u)[R * C]) {
             for (int c = 0; c < C; ++c) u[r * C + c] = t[c];
         }
     }
-}
-
-PTF_DEV void l2_prefetch_bulk(const void *p, unsigned bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
 // ---- pass A ---------------------------------------------------------------------------------------------------
