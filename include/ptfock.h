@@ -111,9 +111,10 @@ int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const void *psi, 
 
 /* Same as ptfock_apply but phi, psi, out are HOST pointers (pinned memory gives full PCIe speed;
  * pageable works).  The library copies Phi (and Psi) to device buffers it owns, applies, copies the
- * result back, and synchronises `stream`.  The copies run on a stream of the plan's, in chunks of block_i
- * orbitals, each wave waiting only for the chunks it reads, so most of the transfer overlaps the kernels.
- * n_targets <= max_targets. */
+ * result back, and synchronises `stream`.  The copies run on a stream of the plan's: Phi in chunks of block_i
+ * orbitals, Psi in chunks of block_j targets, each wave waiting only for the chunks it reads; every block_j
+ * targets of the result start their way back as soon as the last block of orbitals has been accumulated into
+ * them, so nearly all of the transfer overlaps the kernels.  n_targets <= max_targets. */
 int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const void *psi_host, int32_t self_offset,
                       int32_t n_targets, void *out_host, void *stream);
 

@@ -714,21 +714,43 @@ int check_apply_args(const ptfock_plan *p, const void *phi, const void *psi, int
     return PTFOCK_OK;
 }
 
-// Host path (ptfock_apply_host): Phi is copied in chunks of `chunk` orbitals on the plan's copy stream, one event per
-// chunk; a wave waits only for the chunks it reads, so the copy of the rest overlaps the first waves.
+// Host path (ptfock_apply_host): Phi is copied in chunks of `chunk` orbitals and Psi in chunks of `jchunk` targets on
+// the plan's copy stream, one event per chunk; a wave waits only for the chunks it reads, so the copy of the rest
+// overlaps the first waves.  The result goes back the same way: when the last i block has accumulated into a j-block
+// of `out`, that block is final and its device-to-host copy is queued on the copy stream behind an event, so it
+// overlaps the remaining waves (only the last block's copy is exposed).
 struct HostPipe {
     cudaStream_t cs;
-    std::vector<cudaEvent_t> *ev;       // [0, n_chunks): Phi chunk landed; [n_chunks]: Psi landed; [n_chunks + 1]: scratch event
+    std::vector<cudaEvent_t> *ev;       // [0, n_chunks): Phi chunk landed; [n_chunks]: fork event;
+                                        // [psi_base, psi_base + n_jchunks): Psi chunk landed; [out_base, ...): out block final
     int chunk, n_chunks;
-    std::vector<char> waited;
+    int jchunk, n_jchunks, psi_base, out_base;
+    std::vector<char> waited, waited_psi;
+    cd *out_host;                       // host destination of the result (streamed back block by block)
+    size_t gbytes;
+    bool out_streamed;                  // apply_device queued every block of `out`
     cudaError_t err = cudaSuccess;
+    void note(cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; }
     void need(cudaStream_t st, int lo, int hi) {                  // orbitals [lo, hi) of Phi
         for (int c = lo / chunk; c <= (hi - 1) / chunk && c < n_chunks; ++c)
             if (!waited[c]) {
-                const cudaError_t e = cudaStreamWaitEvent(st, (*ev)[c], 0);
-                if (e != cudaSuccess && err == cudaSuccess) err = e;
+                note(cudaStreamWaitEvent(st, (*ev)[c], 0));
                 waited[c] = 1;
             }
+    }
+    void need_psi(cudaStream_t st, int lo, int hi) {              // targets [lo, hi) of Psi
+        for (int c = lo / jchunk; c <= (hi - 1) / jchunk && c < n_jchunks; ++c)
+            if (!waited_psi[c]) {
+                note(cudaStreamWaitEvent(st, (*ev)[psi_base + c], 0));
+                waited_psi[c] = 1;
+            }
+    }
+    void emit_out(cudaStream_t st, const cd *out_dev, int j0, int nj) {   // out[j0, j0 + nj) is final on `st`
+        cudaEvent_t e = (*ev)[out_base + j0 / jchunk];
+        note(cudaEventRecord(e, st));
+        note(cudaStreamWaitEvent(cs, e, 0));
+        note(cudaMemcpyAsync(out_host + (size_t)j0 * (gbytes / sizeof(cd)), out_dev + (size_t)j0 * (gbytes / sizeof(cd)),
+                             gbytes * nj, cudaMemcpyDeviceToHost, cs));
     }
 };
 
@@ -772,7 +794,7 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
     const int n_occ = p->d.n_occ;
     const bool symmetric = (!psi) && self_offset == 0 && n_targets == n_occ && p->v_even && n_occ > 1 && !p->onchip;
     if (p->onchip) {
-        if (hp) { hp->need(st, 0, n_occ); if (psi) w.note(cudaStreamWaitEvent(st, (*hp->ev)[hp->n_chunks], 0)); }
+        if (hp) { hp->need(st, 0, n_occ); if (psi) hp->need_psi(st, 0, n_targets); }
         apply_onchip(p, phi, phi, 1, 0, n_occ, psi ? psi : phi + (size_t)self_offset * p->N, n_targets, out, st, w);
         if (hp) w.note(hp->err);
         w.note(cudaGetLastError());
@@ -806,18 +828,22 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
         const cd *tgt = psi ? psi : phi + (size_t)self_offset * p->N;
         if (hp) {
             // host path: i blocks outermost, so every chunk of Phi is used by all j-blocks as soon as it has landed
-            // and the rest of the copy hides behind those waves (out_j accumulates over the waves in any order)
-            if (psi) w.note(cudaStreamWaitEvent(st, (*hp->ev)[hp->n_chunks], 0));
-            else hp->need(st, self_offset, self_offset + n_targets);
+            // and the rest of the copy hides behind those waves (out_j accumulates over the waves in any order);
+            // during the last i block every finished j-block of `out` starts its way back to the host
+            if (!psi) hp->need(st, self_offset, self_offset + n_targets);
             for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
                 const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
+                const bool last = i0 + ni >= n_occ;
                 hp->need(st, i0, i0 + ni);
                 for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
                     const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
+                    if (psi) hp->need_psi(st, j0, j0 + nj);
                     wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
                     wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
+                    if (last) hp->emit_out(st, out, j0, nj);
                 }
             }
+            hp->out_streamed = true;
         } else {
             for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
                 const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
@@ -911,39 +937,56 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     hp.cs = plan->copy_stream;
     hp.chunk = plan->Ib;
     hp.n_chunks = (plan->d.n_occ + hp.chunk - 1) / hp.chunk;
+    hp.jchunk = plan->Jb;
+    hp.n_jchunks = (n_targets + hp.jchunk - 1) / hp.jchunk;
+    hp.psi_base = hp.n_chunks + 1;
+    hp.out_base = hp.psi_base + hp.n_jchunks;
+    hp.out_host = (cd *)out_host;
+    hp.gbytes = gbytes;
+    hp.out_streamed = false;
     if (!plan->copy_ev) plan->copy_ev = new std::vector<cudaEvent_t>();
-    while ((int)plan->copy_ev->size() < hp.n_chunks + 2) {
+    while ((int)plan->copy_ev->size() < hp.out_base + hp.n_jchunks) {
         cudaEvent_t e;
         CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
         plan->copy_ev->push_back(e);
     }
     hp.ev = plan->copy_ev;
     hp.waited.assign(hp.n_chunks, 0);
+    hp.waited_psi.assign(hp.n_jchunks, 0);
     CU(begin_call(plan, st));
-    // the copy stream starts after whatever the caller queued on `stream` (the event slot [n_chunks + 1] is free here)
-    CU(cudaEventRecord((*hp.ev)[hp.n_chunks + 1], st));
-    CU(cudaStreamWaitEvent(hp.cs, (*hp.ev)[hp.n_chunks + 1], 0));
+    // the copy stream starts after whatever the caller queued on `stream`
+    CU(cudaEventRecord((*hp.ev)[hp.n_chunks], st));
+    CU(cudaStreamWaitEvent(hp.cs, (*hp.ev)[hp.n_chunks], 0));
     // from here on async copies out of the caller's host buffers may be in flight: every exit drains the copy stream
 #define CUH(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_cuda = (int)e__; cudaStreamSynchronize(hp.cs); \
         cudaStreamSynchronize(st); return PTFOCK_ERR_CUDA; } } while (0)
-    if (psi_host) {
-        CUH(cudaMemcpyAsync(plan->st_psi, psi_host, gbytes * n_targets, cudaMemcpyHostToDevice, hp.cs));
-        CUH(cudaEventRecord((*hp.ev)[hp.n_chunks], hp.cs));
-    }
-    // chunks that hold the targets (Psi = Phi[self_offset...]) go first, the rest in the order the i loop reads them
+    auto copy_psi = [&](int c) -> cudaError_t {
+        const int lo = c * hp.jchunk, cnt = (n_targets - lo < hp.jchunk) ? n_targets - lo : hp.jchunk;
+        cudaError_t e = cudaMemcpyAsync(plan->st_psi + (size_t)lo * plan->N, (const cd *)psi_host + (size_t)lo * plan->N, gbytes * cnt,
+                                        cudaMemcpyHostToDevice, hp.cs);
+        return e != cudaSuccess ? e : cudaEventRecord((*hp.ev)[hp.psi_base + c], hp.cs);
+    };
+    auto copy_phi = [&](int c) -> cudaError_t {
+        const int lo = c * hp.chunk, cnt = (plan->d.n_occ - lo < hp.chunk) ? plan->d.n_occ - lo : hp.chunk;
+        cudaError_t e = cudaMemcpyAsync(plan->st_phi + (size_t)lo * plan->N, (const cd *)phi_host + (size_t)lo * plan->N, gbytes * cnt,
+                                        cudaMemcpyHostToDevice, hp.cs);
+        return e != cudaSuccess ? e : cudaEventRecord((*hp.ev)[c], hp.cs);
+    };
+    // copy order = the order the waves read: the first j-block of Psi and the first chunk of Phi, the rest of Psi (the
+    // first i block sweeps all j-blocks), then the rest of Phi.  Psi = Phi[self_offset ...]: the chunks that hold the
+    // targets go first.
     std::vector<int> order;
     const int t_lo = psi_host ? 0 : self_offset / hp.chunk, t_hi = psi_host ? -1 : (self_offset + n_targets - 1) / hp.chunk;
     for (int c = t_lo; c <= t_hi; ++c) order.push_back(c);
     for (int c = 0; c < hp.n_chunks; ++c) if (c < t_lo || c > t_hi) order.push_back(c);
-    for (int c : order) {
-        const int lo = c * hp.chunk, cnt = (plan->d.n_occ - lo < hp.chunk) ? plan->d.n_occ - lo : hp.chunk;
-        CUH(cudaMemcpyAsync(plan->st_phi + (size_t)lo * plan->N, (const cd *)phi_host + (size_t)lo * plan->N, gbytes * cnt,
-                           cudaMemcpyHostToDevice, hp.cs));
-        CUH(cudaEventRecord((*hp.ev)[c], hp.cs));
-    }
+    if (psi_host) CUH(copy_psi(0));
+    size_t first = 0;
+    if (psi_host && !order.empty()) { CUH(copy_phi(order[0])); first = 1; }
+    if (psi_host) for (int c = 1; c < hp.n_jchunks; ++c) CUH(copy_psi(c));
+    for (size_t k = first; k < order.size(); ++k) CUH(copy_phi(order[k]));
     rc = apply_device(plan, plan->st_phi, psi_host ? plan->st_psi : nullptr, self_offset, n_targets, plan->st_out, st, &hp);
     if (rc != PTFOCK_OK) { cudaStreamSynchronize(hp.cs); cudaStreamSynchronize(st); return rc; }
-    CUH(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
+    if (!hp.out_streamed) CUH(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
     CUH(end_call(plan, st));
     CUH(cudaStreamSynchronize(st));
     CUH(cudaStreamSynchronize(hp.cs));

@@ -128,6 +128,16 @@ def test_host_path_and_stream(cuda_device):
             torch.cuda.synchronize()
             assert sym == (1 if nt == 7 else 0)
             assert torch.equal(host, dev.cpu()), (off, nt)
+        # separate Psi through the host path: Psi arrives in chunks of block_j targets, `out` leaves block by block
+        # during the last i block (ragged last chunks on both sides); a second call reuses the events
+        psi2 = synth.random_orbitals(cfg2, 4, 5, cuda_device)
+        hpsi = psi2.cpu().pin_memory()
+        dev = plan.apply(phi2, psi2)
+        for _ in range(2):
+            host = plan.apply_host(hphi, hpsi)
+            assert torch.equal(host, dev.cpu())
+        host1 = plan.apply_host(hphi, hpsi[:1].contiguous().pin_memory())
+        assert torch.equal(host1, dev[:1].cpu())
 
 
 def test_edge_cases_and_errors(cuda_device):
