@@ -390,7 +390,7 @@ def main():
     ap.add_argument("--block-i", type=int, default=0)
     ap.add_argument("--block-j", type=int, default=0)
     ap.add_argument("--workspace-gb", type=float, default=0.0)
-    ap.add_argument("--flags", type=int, default=0, help="ptfock_desc.flags (1 = three-stage slab passes)")
+    ap.add_argument("--flags", type=int, default=0, help="ptfock_desc.flags (1 = three-stage slab passes, 2 = single stream: one wave in flight)")
     ap.add_argument("--targets", type=int, default=0, help="restrict the step to the first T targets (profiling slices)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -84,7 +84,12 @@ enum {
     /* use the three-pass path (slab passes + pencil pass through the pair scratch) even where a grid has a faster
      * dedicated path (64^3: pass8.cuh, 16^3: onchip16.cuh): same results, kept for A/B timing and as a second
      * implementation the tests compare with the oracle */
-    PTFOCK_FLAG_THREE_STAGE_SLABS = 1u
+    PTFOCK_FLAG_THREE_STAGE_SLABS = 1u,
+    /* keep every wave on the caller's stream.  By default, when the scratch bound allows two waves, the general
+     * (non-symmetric) schedule runs the j-blocks with an odd index on a stream of the plan's, in a second scratch slot,
+     * forked from and joined to `stream` inside the call: one wave's kernels fill the SMs while the other's drain.
+     * Same results bit for bit; kept for A/B timing. */
+    PTFOCK_FLAG_SINGLE_STREAM = 2u
 };
 
 /* Builds the plan: v(G) table (with -alpha/N folded in, stored in the kernels' digit-permuted
@@ -182,8 +187,9 @@ int ptfock_last_cuda_error(void);
  *   info[0] = block_i, info[1] = block_j in use, info[2] = scratch bytes, info[3] = kernel launches
  *   issued by the most recent apply, info[4] = pair-solves executed by the most recent apply,
  *   info[5] = 1 if the most recent apply used the symmetric schedule, info[6] = total launches since create,
- *   info[7] = kernel family: 0 three-stage slab passes + pencil pass, 1 two-stage slab passes + 32 x 32 pencil pass
- *             (64^3), 2 single-pass on-chip kernel (16^3). */
+ *   info[7] = kernel family in the low 4 bits: 0 three-stage slab passes + pencil pass, 1 two-stage slab passes +
+ *             32 x 32 pencil pass (64^3), 2 single-pass on-chip kernel (16^3); bit 4 (value 16) set if the scratch
+ *             holds two waves (two waves in flight on the general schedule). */
 int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]);
 
 /* Test hook: W = IFFT[v' * FFT(conj(phi_i) psi_j)] for ONE pair through the same three kernels,

@@ -19,6 +19,7 @@ KERNEL_COULOMB = 0
 KERNEL_HSE = 1
 KERNEL_KINETIC = 2
 FLAG_THREE_STAGE_SLABS = 1
+FLAG_SINGLE_STREAM = 2
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
@@ -314,7 +315,7 @@ class Plan:
         a = (ctypes.c_int64 * 8)()
         _check(lib().ptfock_plan_info(self._h, a), "ptfock_plan_info")
         return {"block_i": a[0], "block_j": a[1], "scratch_bytes": a[2], "last_launches": a[3], "last_pairs": a[4],
-                "last_symmetric": a[5], "total_launches": a[6], "pass8": a[7]}
+                "last_symmetric": a[5], "total_launches": a[6], "pass8": a[7] & 15, "slots": 1 + ((a[7] >> 4) & 1)}
 
     def set_profiling(self, on: bool):
         _check(lib().ptfock_set_profiling(self._h, 1 if on else 0), "ptfock_set_profiling")

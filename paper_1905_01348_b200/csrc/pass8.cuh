@@ -366,6 +366,7 @@ struct P8MidArgs {
     const cd *tw0;       // exp(-2 pi i t / N0)
     int n_pairs;         // pairs in the wave
     int tri_nj;          // > 0: diagonal block of the symmetric schedule, pair = i*tri_nj + j exists only for i <= j
+    int pair0;           // pair index (in the scratch the tensor map covers) of the wave's first pair
 };
 
 PTF_DEV void tensor_g2s_2d_sw(void *dst_smem, const CUtensorMap *map, int c0, int c1, unsigned long long *bar) {
@@ -409,7 +410,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
             if (blockIdx.y * GB + k < g.n_pairs &&
                 !(g.tri_nj > 0 && (int)(blockIdx.y * GB + k) / g.tri_nj > (int)(blockIdx.y * GB + k) % g.tri_nj)) {
                 mbar_expect_tx(&bars[k], S::TILE_B);
-                tensor_g2s_2d_sw(smem_b + k * S::TILE_B, &map, grp_pos * (P * RQ * 2), (blockIdx.y * GB + k) * S::ROWS, &bars[k]);
+                tensor_g2s_2d_sw(smem_b + k * S::TILE_B, &map, grp_pos * (P * RQ * 2), (g.pair0 + blockIdx.y * GB + k) * S::ROWS, &bars[k]);
             }
     }
     // stage 1 / 3 task: (b0 = x0 mod 32, p); element (a0, q, r) at row q*N0 + a0*32 + b0, chunk (p*RQ + r) ^ (b0 & 7)
@@ -496,7 +497,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
     fence_proxy_async();
     group_sync();
     if (tid == 0) {
-        tensor_s2g_2d_sw(&map, grp_pos * (P * RQ * 2), pair * S::ROWS, s);
+        tensor_s2g_2d_sw(&map, grp_pos * (P * RQ * 2), (g.pair0 + pair) * S::ROWS, s);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // shared memory must outlive the store's reads
     }

@@ -37,6 +37,7 @@ struct PencilTmaArgs {
     const cd *tw0;
     int slab_pts;
     int tri_nj;          // see PencilArgs
+    int pair0;           // pair index (in the scratch the tensor map covers) of the wave's first pair
 };
 
 // grid = (ceil(slab_pts / CW), pairs); the tensor map views the scratch as [pairs*N0 rows][2*slab_pts doubles]
@@ -53,7 +54,7 @@ pencil_tma(const __grid_constant__ CUtensorMap map, const PencilTmaArgs g) {
     const long long sp = g.slab_pts;
     if (g.tri_nj > 0 && (int)blockIdx.y / g.tri_nj > (int)blockIdx.y % g.tri_nj) return;
     const int p0 = blockIdx.x * CW;
-    const int row0 = blockIdx.y * N0;
+    const int row0 = (g.pair0 + blockIdx.y) * N0;
     if (tid == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

@@ -202,6 +202,12 @@ struct ptfock_plan {
     cd *scratch;
     size_t scratch_bytes;
     int Ib, Jb;
+    // two waves in flight (general schedule): the scratch holds `slots` waves of Ib * Jb pair densities; waves of
+    // j-blocks with an odd index run on aux_stream in the second slot, so one wave's passes fill the SMs while the
+    // other wave's kernel drains (the tail of a launch is one CTA lifetime long, ~20 % of pass A)
+    int slots;
+    cudaStream_t aux_stream;
+    cudaEvent_t fork_ev, join_ev;
     bool v_even;
     const SlabEntry *slab;
     const PencilEntry *pencil;
@@ -266,6 +272,9 @@ void free_plan(ptfock_plan *p) {
     cudaFree(p->chol_info);
     if (p->chol_info_host) cudaFreeHost(p->chol_info_host);
     if (p->busy_ev) cudaEventDestroy(p->busy_ev);
+    if (p->fork_ev) cudaEventDestroy(p->fork_ev);
+    if (p->join_ev) cudaEventDestroy(p->join_ev);
+    if (p->aux_stream) cudaStreamDestroy(p->aux_stream);
     if (p->ev_pool) { for (cudaEvent_t e : *p->ev_pool) cudaEventDestroy(e); delete p->ev_pool; }
     if (p->copy_ev) { for (cudaEvent_t e : *p->copy_ev) cudaEventDestroy(e); delete p->copy_ev; }
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
@@ -495,20 +504,31 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
         dense_min = sizeof(cd) * (npad * npad + npad + ks * nmax * nmax);
     }
     // a failing allocation (fragmentation, another allocator holding the memory) shrinks the wave instead of failing
+    // a second slot (two waves in flight) if it fits the bound
+    int slots = (!(d.flags & PTFOCK_FLAG_SINGLE_STREAM) && !p->onchip && 2 * (size_t)Ib * Jb * pair_bytes <= limit &&
+                 2LL * Ib * Jb <= 65535) ? 2 : 1;
     for (;;) {
-        p->scratch_bytes = std::max((size_t)Ib * Jb * pair_bytes, dense_min);
+        p->scratch_bytes = std::max((size_t)slots * Ib * Jb * pair_bytes, dense_min);
         cudaError_t e = cudaMalloc(&p->scratch, p->scratch_bytes);
         if (e == cudaSuccess) break;
         cudaGetLastError();
         p->scratch = nullptr;
-        if (e != cudaErrorMemoryAllocation || d.workspace_bytes || (Ib == 1 && Jb == 1)) {
+        if (e != cudaErrorMemoryAllocation || (slots == 1 && (d.workspace_bytes || (Ib == 1 && Jb == 1)))) {
             g_last_cuda = (int)e; free_plan(p); return PTFOCK_ERR_ALLOC;
         }
-        if (Ib > 1) Ib = (Ib + 1) / 2; else Jb = (Jb + 1) / 2;
+        if (slots == 2) slots = 1;
+        else if (Ib > 1) Ib = (Ib + 1) / 2;
+        else Jb = (Jb + 1) / 2;
     }
     p->Ib = Ib;
     p->Jb = Jb;
+    p->slots = slots;
     CUP(cudaEventCreateWithFlags(&p->busy_ev, cudaEventDisableTiming));
+    if (slots == 2) {
+        CUP(cudaStreamCreateWithFlags(&p->aux_stream, cudaStreamNonBlocking));
+        CUP(cudaEventCreateWithFlags(&p->fork_ev, cudaEventDisableTiming));
+        CUP(cudaEventCreateWithFlags(&p->join_ev, cudaEventDisableTiming));
+    }
     p->use_tma = 0;
     {
         typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -522,7 +542,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
         if (p8) {
             // scratch as [pairs * nq * n0 rows][2 * qpts doubles]; box = 128 bytes x all (q, x0) rows of one pair
             if (!have) { free_plan(p); return PTFOCK_ERR_CUDA; }
-            const cuuint64_t dims[2] = { (cuuint64_t)2 * p8->qpts, (cuuint64_t)Ib * Jb * p8->rows };
+            const cuuint64_t dims[2] = { (cuuint64_t)2 * p8->qpts, (cuuint64_t)slots * Ib * Jb * p8->rows };
             const cuuint64_t strides[1] = { (cuuint64_t)p8->qpts * sizeof(cd) };
             const cuuint32_t box[2] = { (cuuint32_t)(2 * p8->p * p8->rq), (cuuint32_t)p8->rows };
             CUresult r = ((encode_fn)fn)(&p->tmap8, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
@@ -531,7 +551,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
             if (r != CUDA_SUCCESS) { g_last_cuda = (int)r; free_plan(p); return PTFOCK_ERR_CUDA; }
         } else if (pencil->run_tma) {
             if (!have) { free_plan(p); return PTFOCK_ERR_CUDA; }
-            const cuuint64_t dims[2] = { (cuuint64_t)2 * p->slab_pts, (cuuint64_t)Ib * Jb * d.n[0] };
+            const cuuint64_t dims[2] = { (cuuint64_t)2 * p->slab_pts, (cuuint64_t)slots * Ib * Jb * d.n[0] };
             const cuuint64_t strides[1] = { (cuuint64_t)p->slab_pts * sizeof(cd) };
             const cuuint32_t box[2] = { (cuuint32_t)(2 * pencil->tma_cw), (cuuint32_t)d.n[0] };
             CUresult r = ((encode_fn)fn)(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->scratch, dims, strides, box, estr,
@@ -584,7 +604,7 @@ extern "C" int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]) {
     info[4] = plan->last_pairs;
     info[5] = plan->last_symmetric;
     info[6] = plan->total_launches;
-    info[7] = plan->onchip ? 2 : (plan->p8 ? 1 : 0);
+    info[7] = (plan->onchip ? 2 : (plan->p8 ? 1 : 0)) | (plan->slots == 2 ? 16 : 0);
     return PTFOCK_OK;
 }
 
@@ -595,10 +615,15 @@ namespace {
 
 struct Wave {
     ptfock_plan *p;
-    cudaStream_t st;
+    cudaStream_t st;                    // the stream the next wave's launches go to (the caller's, or the plan's aux stream)
     long long launches, pairs;
     cudaError_t err;                    // first failure of an event / wait / launch in this call
+    cudaStream_t st0 = nullptr;         // the caller's stream
+    int slot = 0;                       // scratch slot of the next wave
     void note(cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; }
+    void use(int s) { slot = s; st = s ? p->aux_stream : st0; }
+    long long pair0() const { return (long long)slot * p->Ib * p->Jb; }
+    cd *scratch() const { return p->scratch + (size_t)pair0() * (size_t)p->N; }
 };
 
 // every call that touches the plan's buffers starts with begin_call and ends with end_call: a call on another stream
@@ -635,7 +660,7 @@ void mark(Wave &w, int tag) {
 void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int j0, int nj, int tri = 0) {
     ptfock_plan *p = w.p;
     SlabArgs a;
-    a.a = phi; a.b = psi; a.scratch = p->scratch; a.out = nullptr;
+    a.a = phi; a.b = psi; a.scratch = w.scratch(); a.out = nullptr;
     a.tw1 = p->tw_dev[1]; a.tw2 = p->tw_dev[2];
     a.grid_pts = p->N; a.n0 = p->d.n[0];
     a.a0 = i0; a.na = ni; a.b0 = j0;
@@ -651,7 +676,7 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
         mark(w, 0);
         P8MidArgs b;
         b.v = p->v8_dev; b.tw0 = p->tw_dev[0];
-        b.n_pairs = ni * nj; b.tri_nj = tri ? nj : 0;
+        b.n_pairs = ni * nj; b.tri_nj = tri ? nj : 0; b.pair0 = (int)w.pair0();
         p->p8->mid(p->tmap8, b, ni * nj, w.st);
         mark(w, 1);
         w.launches += 2;
@@ -662,11 +687,11 @@ void wave_forward_mid(Wave &w, const cd *phi, const cd *psi, int i0, int ni, int
     mark(w, 0);
     if (p->use_tma) {
         PencilTmaArgs b;
-        b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts; b.tri_nj = tri ? nj : 0;
+        b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts; b.tri_nj = tri ? nj : 0; b.pair0 = (int)w.pair0();
         p->pencil->run_tma(p->tmap, b, ni * nj, w.st);
     } else {
         PencilArgs b;
-        b.scratch = p->scratch; b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts; b.tri_nj = tri ? nj : 0;
+        b.scratch = w.scratch(); b.v = p->v_dev; b.tw0 = p->tw_dev[0]; b.slab_pts = p->slab_pts; b.tri_nj = tri ? nj : 0;
         p->pencil->run(b, ni * nj, w.st);
     }
     mark(w, 1);
@@ -679,7 +704,7 @@ void wave_accumulate(Wave &w, const cd *orb, int s0, int ns, cd *out, int t0, in
                      int conj_w, int tri = 0) {
     ptfock_plan *p = w.p;
     SlabArgs a;
-    a.a = orb; a.b = nullptr; a.scratch = p->scratch; a.out = out;
+    a.a = orb; a.b = nullptr; a.scratch = w.scratch(); a.out = out;
     a.tw1 = p->tw_dev[1]; a.tw2 = p->tw_dev[2];
     a.grid_pts = p->N; a.n0 = p->d.n[0];
     a.a0 = s0; a.na = ns; a.b0 = t0;
@@ -725,24 +750,24 @@ struct HostPipe {
                                         // [psi_base, psi_base + n_jchunks): Psi chunk landed; [out_base, ...): out block final
     int chunk, n_chunks;
     int jchunk, n_jchunks, psi_base, out_base;
-    std::vector<char> waited, waited_psi;
+    std::vector<char> waited[2], waited_psi[2];      // per stream (slot) of the two-wave schedule
     cd *out_host;                       // host destination of the result (streamed back block by block)
     size_t gbytes;
     bool out_streamed;                  // apply_device queued every block of `out`
     cudaError_t err = cudaSuccess;
     void note(cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; }
-    void need(cudaStream_t st, int lo, int hi) {                  // orbitals [lo, hi) of Phi
+    void need(cudaStream_t st, int slot, int lo, int hi) {        // orbitals [lo, hi) of Phi, for the waves of `slot` on `st`
         for (int c = lo / chunk; c <= (hi - 1) / chunk && c < n_chunks; ++c)
-            if (!waited[c]) {
+            if (!waited[slot][c]) {
                 note(cudaStreamWaitEvent(st, (*ev)[c], 0));
-                waited[c] = 1;
+                waited[slot][c] = 1;
             }
     }
-    void need_psi(cudaStream_t st, int lo, int hi) {              // targets [lo, hi) of Psi
+    void need_psi(cudaStream_t st, int slot, int lo, int hi) {    // targets [lo, hi) of Psi
         for (int c = lo / jchunk; c <= (hi - 1) / jchunk && c < n_jchunks; ++c)
-            if (!waited_psi[c]) {
+            if (!waited_psi[slot][c]) {
                 note(cudaStreamWaitEvent(st, (*ev)[psi_base + c], 0));
-                waited_psi[c] = 1;
+                waited_psi[slot][c] = 1;
             }
     }
     void emit_out(cudaStream_t st, const cd *out_dev, int j0, int nj) {   // out[j0, j0 + nj) is final on `st`
@@ -791,10 +816,11 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
     if (overlaps(out, gbytes * n_targets, phi, gbytes * p->d.n_occ)) return PTFOCK_ERR_ALIAS;
     if (psi && overlaps(out, gbytes * n_targets, psi, gbytes * n_targets)) return PTFOCK_ERR_ALIAS;
     Wave w{ p, st, 0, 0, cudaSuccess };
+    w.st0 = st;
     const int n_occ = p->d.n_occ;
     const bool symmetric = (!psi) && self_offset == 0 && n_targets == n_occ && p->v_even && n_occ > 1 && !p->onchip;
     if (p->onchip) {
-        if (hp) { hp->need(st, 0, n_occ); if (psi) hp->need_psi(st, 0, n_targets); }
+        if (hp) { hp->need(st, 0, 0, n_occ); if (psi) hp->need_psi(st, 0, 0, n_targets); }
         apply_onchip(p, phi, phi, 1, 0, n_occ, psi ? psi : phi + (size_t)self_offset * p->N, n_targets, out, st, w);
         if (hp) w.note(hp->err);
         w.note(cudaGetLastError());
@@ -810,12 +836,13 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
         // square blocks; block pair (bi <= bj): W_ij for i in bi, j in bj serves out_j (as is) and, off the
         // diagonal, out_i through W_ji = conj(W_ij) (v real and even).
         int bs = p->Ib < p->Jb ? p->Ib : p->Jb;
-        while ((size_t)(bs * 2) * (bs * 2) * gbytes <= p->scratch_bytes && bs * 2 <= n_occ && (bs * 2) * (bs * 2) <= 65535) bs *= 2;
+        while ((size_t)(bs * 2) * (bs * 2) * gbytes <= p->scratch_bytes && bs * 2 <= n_occ && (bs * 2) * (bs * 2) <= 65535 &&
+               (long long)(bs * 2) * (bs * 2) <= (long long)p->slots * p->Ib * p->Jb) bs *= 2;      // (the tensor maps cover slots*Ib*Jb pairs)
         for (int j0 = 0; j0 < n_occ; j0 += bs) {
             const int nj = (n_occ - j0 < bs) ? n_occ - j0 : bs;
             for (int i0 = 0; i0 <= j0; i0 += bs) {
                 const int ni = (n_occ - i0 < bs) ? n_occ - i0 : bs;
-                if (hp) { hp->need(st, i0, i0 + ni); hp->need(st, j0, j0 + nj); }
+                if (hp) { hp->need(st, 0, i0, i0 + ni); hp->need(st, 0, j0, j0 + nj); }
                 // diagonal blocks (i0 == j0): only the pairs i <= j are solved; W_ij then serves out_j (loop i <= j) and,
                 // through conj, out_i (loop j > i)
                 const int tri = (i0 == j0) ? 1 : 0;
@@ -826,33 +853,48 @@ int apply_device(ptfock_plan *p, const cd *phi, const cd *psi, int self_offset, 
         }
     } else {
         const cd *tgt = psi ? psi : phi + (size_t)self_offset * p->N;
+        // two waves in flight: j-blocks with an odd index run on the plan's aux stream in the second scratch slot.  A
+        // j-block always runs on the same stream, so the read-modify-writes of its `out` stay ordered; the two streams
+        // never touch the same targets.  (Per-pass profiling keeps everything on the caller's stream.)
+        const bool dual = p->slots == 2 && !p->profiling && n_targets > p->Jb;
+        if (dual) {
+            w.note(cudaEventRecord(p->fork_ev, st));
+            w.note(cudaStreamWaitEvent(p->aux_stream, p->fork_ev, 0));
+        }
         if (hp) {
             // host path: i blocks outermost, so every chunk of Phi is used by all j-blocks as soon as it has landed
             // and the rest of the copy hides behind those waves (out_j accumulates over the waves in any order);
             // during the last i block every finished j-block of `out` starts its way back to the host
-            if (!psi) hp->need(st, self_offset, self_offset + n_targets);
             for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
                 const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
                 const bool last = i0 + ni >= n_occ;
-                hp->need(st, i0, i0 + ni);
                 for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
                     const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
-                    if (psi) hp->need_psi(st, j0, j0 + nj);
+                    w.use(dual ? (j0 / p->Jb) & 1 : 0);
+                    hp->need(w.st, w.slot, i0, i0 + ni);
+                    if (psi) hp->need_psi(w.st, w.slot, j0, j0 + nj);
+                    else hp->need(w.st, w.slot, self_offset + j0, self_offset + j0 + nj);
                     wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
                     wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
-                    if (last) hp->emit_out(st, out, j0, nj);
+                    if (last) hp->emit_out(w.st, out, j0, nj);
                 }
             }
             hp->out_streamed = true;
         } else {
             for (int j0 = 0; j0 < n_targets; j0 += p->Jb) {
                 const int nj = (n_targets - j0 < p->Jb) ? n_targets - j0 : p->Jb;
+                w.use(dual ? (j0 / p->Jb) & 1 : 0);
                 for (int i0 = 0; i0 < n_occ; i0 += p->Ib) {
                     const int ni = (n_occ - i0 < p->Ib) ? n_occ - i0 : p->Ib;
                     wave_forward_mid(w, phi, tgt, i0, ni, j0, nj);
                     wave_accumulate(w, phi, i0, ni, out, j0, nj, nj, 1, 0);
                 }
             }
+        }
+        w.use(0);
+        if (dual) {
+            w.note(cudaEventRecord(p->join_ev, p->aux_stream));
+            w.note(cudaStreamWaitEvent(st, p->join_ev, 0));
         }
     }
     if (hp) w.note(hp->err);
@@ -951,8 +993,7 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
         plan->copy_ev->push_back(e);
     }
     hp.ev = plan->copy_ev;
-    hp.waited.assign(hp.n_chunks, 0);
-    hp.waited_psi.assign(hp.n_jchunks, 0);
+    for (int k = 0; k < 2; ++k) { hp.waited[k].assign(hp.n_chunks, 0); hp.waited_psi[k].assign(hp.n_jchunks, 0); }
     CU(begin_call(plan, st));
     // the copy stream starts after whatever the caller queued on `stream`
     CU(cudaEventRecord((*hp.ev)[hp.n_chunks], st));
@@ -1007,6 +1048,7 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
         fill_ones<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(plan->ones, plan->N);
     }
     Wave w{ plan, st, 0, 0, cudaSuccess };
+    w.st0 = st;
     if (plan->onchip) {
         apply_onchip(plan, (const cd *)phi_i, plan->ones, 0, 0, 1, (const cd *)psi_j, 1, (cd *)w_out, st, w);
     } else {
