@@ -209,6 +209,10 @@ int ptfock_get_profile(ptfock_plan *plan, double ms[3], int64_t launches[3], int
  * stream, synchronous, ~50 ms) and writes the best sustained rate in TFLOP/s (2 flops per DFMA) to HOST memory. */
 int ptfock_measure_dfma_peak(int32_t device, double *tflops_host);
 
+/* Same for the FP64 tensor pipe (mma.sync m8n8k4, SASS DMMA.8x8x4): the roof of ptfock_overlap / ptfock_rotate /
+ * ptfock_residual / ptfock_orthonormalize, whose contractions run there (csrc/dense_mma.cuh). */
+int ptfock_measure_dmma_peak(int32_t device, double *tflops_host);
+
 /* Measurement aid for the scratch-residency question (SURVEY.md 8(d) "a third roof to watch"):
  * copies `bytes` bytes device-to-device `reps` times back to back with a plain 128-bit grid-stride kernel and
  * writes the best read+write rate in GB/s to HOST memory.  A working set (2 * bytes) well under the L2 size

@@ -23,7 +23,7 @@ FLAG_SINGLE_STREAM = 2
 
 EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_apply_host", "ptfock_destroy",
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
-           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_copy_bandwidth",
+           "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_dmma_peak", "ptfock_measure_copy_bandwidth",
            "ptfock_overlap", "ptfock_rotate", "ptfock_residual", "ptfock_density", "ptfock_orthonormalize",
            "ptfock_hloc_apply", "ptfock_axpby", "ptfock_banddot"]
 
@@ -82,6 +82,7 @@ def lib() -> ctypes.CDLL:
         L.ptfock_set_profiling.argtypes = [vp, i32]
         L.ptfock_get_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64), i32]
         L.ptfock_measure_dfma_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double)]
+        L.ptfock_measure_dmma_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double)]
         L.ptfock_measure_copy_bandwidth.argtypes = [i32, ctypes.c_uint64, i32, ctypes.POINTER(ctypes.c_double)]
         L.ptfock_overlap.argtypes = [vp, vp, i32, vp, i32, vp, vp]
         L.ptfock_rotate.argtypes = [vp, vp, i32, vp, i32, vp, vp]
@@ -348,6 +349,13 @@ def measure_fp64_peak(device: int = 0) -> float:
     """Sustained DFMA rate of the device in TFLOP/s (ptfock_measure_dfma_peak)."""
     v = ctypes.c_double(0.0)
     _check(lib().ptfock_measure_dfma_peak(int(device), ctypes.byref(v)), "ptfock_measure_dfma_peak")
+    return v.value
+
+
+def measure_fp64_tensor_peak(device: int = 0) -> float:
+    """Sustained FP64 tensor-core (DMMA) rate of the device in TFLOP/s (ptfock_measure_dmma_peak)."""
+    v = ctypes.c_double(0.0)
+    _check(lib().ptfock_measure_dmma_peak(int(device), ctypes.byref(v)), "ptfock_measure_dmma_peak")
     return v.value
 
 

@@ -8,6 +8,7 @@
 #include "pass8.cuh"
 #include "onchip16.cuh"
 #include "dense.cuh"
+#include "dense_mma.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -499,8 +500,7 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     size_t dense_min = 0;
     {
         const size_t nmax = (size_t)std::max(d.n_occ, d.max_targets), npad = (nmax + 63) / 64 * 64;
-        const size_t tiles = (npad / 64) * (npad / 64);
-        const size_t ks = std::max<size_t>(1, std::min<size_t>(8, (4 * (size_t)prop.multiProcessorCount + tiles - 1) / tiles));
+        const size_t ks = 8;                                 // overlap_into picks 1 .. 8 splits
         dense_min = sizeof(cd) * (npad * npad + npad + ks * nmax * nmax);
     }
     // a failing allocation (fragmentation, another allocator holding the memory) shrinks the wave instead of failing
@@ -562,6 +562,8 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
             p->use_tma = 1;
         }
     }
+    CUP(cudaFuncSetAttribute(overlap_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, kOverlapMmaSmem));
+    CUP(cudaFuncSetAttribute(rotate_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, kRotateMmaSmem));
     CUP(cudaMalloc(&p->partials, sizeof(double2) * 1024));
     CUP(cudaMalloc(&p->result_dev, sizeof(double2)));
     CUP(cudaMallocHost(&p->result_host, sizeof(double2)));
@@ -1084,17 +1086,27 @@ int check_dev_ptrs(const ptfock_plan *p, std::initializer_list<const void *> ptr
 int overlap_into(ptfock_plan *p, const cd *a, int n_a, const cd *b, int n_b, cd *s, int ld_s, cd *work, size_t work_bytes,
                  cudaStream_t st) {
     const int tiles = ((n_a + kDT - 1) / kDT) * ((n_b + kDT - 1) / kDT);
-    long long ks = (4LL * p->sm_count + tiles - 1) / tiles;
-    ks = std::max(1LL, std::min(ks, p->N / 1024 > 0 ? p->N / 1024 : 1LL));
+    // split K so that the CTAs fill whole rounds of the 2 x sm_count resident CTAs: the split with the least
+    // (rounds / splits) wins, the smaller one on a tie (1024 orbitals: 256 tiles x 8 splits = 6.9 rounds)
     const size_t per = sizeof(cd) * (size_t)n_a * n_b;
-    ks = std::min<long long>(ks, (long long)(work_bytes / per));
-    if (ks < 1) return PTFOCK_ERR_ALLOC;
+    long long ks_max = std::min<long long>(8, p->N / 1024 > 0 ? p->N / 1024 : 1LL);
+    ks_max = std::min<long long>(ks_max, (long long)(work_bytes / per));
+    if (ks_max < 1) return PTFOCK_ERR_ALLOC;
+    long long ks = 1;
+    {
+        const long long slots = 2LL * p->sm_count;
+        double best = 1e300;
+        for (long long c = 1; c <= ks_max; ++c) {
+            const double cost = (double)((tiles * c + slots - 1) / slots) / (double)c;
+            if (cost < best * (1.0 - 1e-9)) { best = cost; ks = c; }
+        }
+    }
     long long pps = (p->N + ks - 1) / ks;
     pps = (pps + kDK - 1) / kDK * kDK;
     ks = (p->N + pps - 1) / pps;
     OverlapArgs g;
     g.a = a; g.b = b; g.part = work; g.n_pts = p->N; g.pts_per_split = pps; g.n_a = n_a; g.n_b = n_b; g.ld = n_b;
-    overlap_partial<<<dim3((n_a + kDT - 1) / kDT, (n_b + kDT - 1) / kDT, (unsigned)ks), 256, 0, st>>>(g);
+    overlap_mma<<<dim3((n_a + kDT - 1) / kDT, (n_b + kDT - 1) / kDT, (unsigned)ks), 128, kOverlapMmaSmem, st>>>(g);
     const long long cnt = (long long)n_a * n_b;
     overlap_reduce<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(work, (int)ks, n_a, n_b, n_b, p->volume / (double)p->N, s, ld_s);
     p->total_launches += 2;
@@ -1102,7 +1114,7 @@ int overlap_into(ptfock_plan *p, const cd *a, int n_a, const cd *b, int n_b, cd 
 }
 
 void rotate_launch(ptfock_plan *p, const RotateArgs &g, cudaStream_t st) {
-    rotate_kernel<<<dim3((unsigned)((g.n_pts + kDT - 1) / kDT), (g.n_out + kDT - 1) / kDT), 256, 0, st>>>(g);
+    rotate_mma<<<dim3((g.n_out + kDT - 1) / kDT, (unsigned)((g.n_pts + kDT - 1) / kDT)), 128, kRotateMmaSmem, st>>>(g);
     p->total_launches += 1;
 }
 
@@ -1360,7 +1372,13 @@ extern "C" int ptfock_banddot(ptfock_plan *plan, const void *a, const void *b, i
     return PTFOCK_OK;
 }
 
-extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
+namespace {
+int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host);
+}
+extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) { return measure_fp64_peak(device, false, tflops_host); }
+extern "C" int ptfock_measure_dmma_peak(int32_t device, double *tflops_host) { return measure_fp64_peak(device, true, tflops_host); }
+namespace {
+int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host) {
     if (!tflops_host) return PTFOCK_ERR_INVALID_ARG;
     GUARD(device);
     cudaDeviceProp prop;
@@ -1375,13 +1393,15 @@ extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
     double best = 0.0;
     for (int rep = 0; rep < 6; ++rep) {             // first repetitions warm the clocks up
         cudaEventRecord(e0, 0);
-        fp64_peak_kernel<<<blocks, 256>>>(sink, iters, 1.0000001, 1e-9);
+        if (tensor) dmma_peak_kernel<<<blocks, 256>>>(sink, iters, 1e-3, 1e-3);
+        else fp64_peak_kernel<<<blocks, 256>>>(sink, iters, 1.0000001, 1e-9);
         cudaEventRecord(e1, 0);
         cudaError_t e = cudaEventSynchronize(e1);
         if (e != cudaSuccess) { g_last_cuda = (int)e; cudaFree(sink); return PTFOCK_ERR_CUDA; }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
-        const double tf = 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+        // per thread and iteration: 8 DFMAs, or 8 warp-wide 8 x 8 x 4 MMAs (256 FMAs shared by 32 lanes = 8 per lane)
+        const double tf = (tensor ? 8.0 : 1.0) * 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
         if (rep >= 2 && tf > best) best = tf;
     }
     cudaEventDestroy(e0);
@@ -1390,6 +1410,7 @@ extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) {
     *tflops_host = best;
     return PTFOCK_OK;
 }
+}  // namespace
 
 extern "C" int ptfock_measure_copy_bandwidth(int32_t device, uint64_t bytes, int32_t reps, double *gbs_host) {
     if (!gbs_host || bytes < 4096 || reps < 1) return PTFOCK_ERR_INVALID_ARG;
