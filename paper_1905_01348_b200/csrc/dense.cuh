@@ -1,8 +1,9 @@
 // dense.cuh -- the dense-algebra neighbours of the Fock exchange path on one GPU:
 // overlap matrices, rotations, the PT-CN residuals, the density, Cholesky + triangular solve orthonormalisation
 // (Sec. 3.3 Alg. 3; Sec. 3.4).  The paper calls cuBLAS / cuSOLVER for these; here they
-// are hand-written fp64 kernels on the plain FP64 pipe (register-tiled, shared-memory staged), all deterministic
-// (split-K partial sums are added in a fixed order, no atomics).
+// are hand-written fp64 kernels, all deterministic (split-K partial sums are added in a fixed order, no atomics).
+// This file: argument structs, reductions, the density, the blocked Cholesky and the triangular-solve blocks (plain
+// FP64 pipe); the two big contractions (overlap, rotation) run on the FP64 tensor cores: dense_mma.cuh.
 //
 // Orbitals are [orbital][grid point] complex fp64, the inner product is (a, b) = w sum_r conj(a(r)) b(r), w = Omega/N.
 #pragma once
@@ -10,73 +11,17 @@
 
 namespace ptfock {
 
-constexpr int kDT = 64;         // output tile edge of the GEMM-like kernels (16 x 16 threads, 4 x 4 complex per thread)
+constexpr int kDT = 64;         // output tile edge of the GEMM-like kernels
 constexpr int kDK = 16;         // contraction step staged through shared memory
 constexpr int kDP = kDK + 1;    // pitch of a [64][16] tile (elements)
 
-// ---- overlap: part[ks][m][n] = sum over this split's points of conj(a[m][r]) b[n][r] -----------------------------------
-// grid = (ceil(n_a / 64), ceil(n_b / 64), k_splits); thread (ty, tx) owns rows m = ty + 16 i and columns n = tx + 16 j:
-// the shared-memory reads of a tile are a broadcast (a) or 16 consecutive pitch-17 rows (b): conflict free.
+// ---- overlap: part[ks][m][n] = sum over this split's points of conj(a[m][r]) b[n][r]   (kernel: overlap_mma) ----------
 struct OverlapArgs {
     const cd *a, *b;
-    cd *part;               // [k_splits][n_a_pad? no: n_a][ld]
+    cd *part;               // [k_splits][n_a][ld]
     long long n_pts, pts_per_split;
     int n_a, n_b, ld;       // ld = row pitch of part / S (>= n_b)
 };
-
-__global__ void __launch_bounds__(256) overlap_partial(const OverlapArgs g) {
-    __shared__ cd As[kDT * kDP], Bs[kDT * kDP];
-    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    const int m0 = blockIdx.x * kDT, n0 = blockIdx.y * kDT;
-    const long long r_beg = (long long)blockIdx.z * g.pts_per_split;
-    const long long r_end = min(g.n_pts, r_beg + g.pts_per_split);
-    cd acc[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
-    // loader: thread t brings points 4 (t % 4) .. + 3 of row t / 4 of both tiles
-    const int lrow = tid >> 2, lk = (tid & 3) * 4;
-    const bool a_ok = m0 + lrow < g.n_a, b_ok = n0 + lrow < g.n_b;
-    const cd *ap = g.a + (long long)(m0 + lrow) * g.n_pts + lk;
-    const cd *bp = g.b + (long long)(n0 + lrow) * g.n_pts + lk;
-    for (long long r = r_beg; r < r_end; r += kDK) {
-        cd av[4], bv[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const bool in = r + lk + q < r_end;
-            av[q] = (a_ok && in) ? ap[r + q] : make_double2(0.0, 0.0);
-            bv[q] = (b_ok && in) ? bp[r + q] : make_double2(0.0, 0.0);
-        }
-        __syncthreads();                                // the previous step's reads are done
-#pragma unroll
-        for (int q = 0; q < 4; ++q) { As[lrow * kDP + lk + q] = av[q]; Bs[lrow * kDP + lk + q] = bv[q]; }
-        __syncthreads();
-#pragma unroll
-        for (int kk = 0; kk < kDK; ++kk) {
-            cd x[4], y[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) x[i] = As[(ty + 16 * i) * kDP + kk];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) y[j] = Bs[(tx + 16 * j) * kDP + kk];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {           // acc += conj(x) y
-                    acc[i][j].x = fma(x[i].x, y[j].x, fma(x[i].y, y[j].y, acc[i][j].x));
-                    acc[i][j].y = fma(x[i].x, y[j].y, fma(-x[i].y, y[j].x, acc[i][j].y));
-                }
-        }
-    }
-    cd *out = g.part + (long long)blockIdx.z * g.n_a * g.ld;
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int m = m0 + ty + 16 * i, n = n0 + tx + 16 * j;
-            if (m < g.n_a && n < g.n_b) out[(long long)m * g.ld + n] = acc[i][j];
-        }
-}
 
 // s[m][n] = w * sum_ks part[ks][m][n] (fixed order)
 __global__ void __launch_bounds__(256) overlap_reduce(const cd *part, int k_splits, int n_a, int n_b, int ld_part, double w,
@@ -98,7 +43,7 @@ __global__ void __launch_bounds__(256) overlap_reduce(const cd *part, int k_spli
 // mode 1: out = h - acc                  (Alg. 1 line 1, R_n = H Psi - Psi S)
 // mode 2: out = p + f (h - acc) - q      (Alg. 3 line 5, R_f; f = i dt / 2)
 // mode 3: out = out - acc                (blocked triangular solve: block column minus the finished columns' part)
-// grid = (ceil(n_pts / 64), ceil(n_out / 64)); thread (ty, tx) owns columns n = ty + 16 i and points r = tx + 16 j.
+// (kernel: rotate_mma)
 struct RotateArgs {
     const cd *a;            // [n_a][n_pts]
     const cd *s;            // coefficients
@@ -109,72 +54,6 @@ struct RotateArgs {
     int n_first;            // first output column (offset into h, p, q, out and into S's column index)
     double fx, fy;          // f
 };
-
-__global__ void __launch_bounds__(256) rotate_kernel(const RotateArgs g) {
-    __shared__ cd As[kDK * kDT], Ss[kDK * (kDT + 1)];
-    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    const long long r0 = (long long)blockIdx.x * kDT;
-    const int n0 = g.n_first + blockIdx.y * kDT, n_end = g.n_first + g.n_out;
-    cd acc[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
-    // loaders: A tile [16 m][64 r]: thread t -> m = t / 16, r = 4 (t % 16) .. + 3;  S tile [16 m][64 n] likewise
-    const int lm = tid >> 4, lc = (tid & 15) * 4;
-    for (int m0 = 0; m0 < g.n_a; m0 += kDK) {
-        cd av[4], sv[4];
-        const bool m_ok = m0 + lm < g.n_a;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            av[q] = (m_ok && r0 + lc + q < g.n_pts) ? g.a[(long long)(m0 + lm) * g.n_pts + r0 + lc + q] : make_double2(0.0, 0.0);
-            const int n = n0 + lc + q;
-            if (m_ok && n < n_end) {
-                sv[q] = g.conj_t ? cconj(g.s[(long long)n * g.ld + m0 + lm]) : g.s[(long long)(m0 + lm) * g.ld + n];
-            } else {
-                sv[q] = make_double2(0.0, 0.0);
-            }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < 4; ++q) { As[lm * kDT + lc + q] = av[q]; Ss[lm * (kDT + 1) + lc + q] = sv[q]; }
-        __syncthreads();
-#pragma unroll
-        for (int kk = 0; kk < kDK; ++kk) {
-            cd x[4], y[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) x[i] = Ss[kk * (kDT + 1) + ty + 16 * i];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) y[j] = As[kk * kDT + tx + 16 * j];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {           // acc += x y
-                    acc[i][j].x = fma(x[i].x, y[j].x, fma(-x[i].y, y[j].y, acc[i][j].x));
-                    acc[i][j].y = fma(x[i].x, y[j].y, fma(x[i].y, y[j].x, acc[i][j].y));
-                }
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int n = n0 + ty + 16 * i;
-            const long long r = r0 + tx + 16 * j;
-            if (n >= n_end || r >= g.n_pts) continue;
-            const long long k = (long long)n * g.n_pts + r;
-            cd v = acc[i][j];
-            if (g.mode == 1) {
-                v = csub(g.h[k], v);
-            } else if (g.mode == 2) {
-                const cd d = csub(g.h[k], v), pv = g.p[k], qv = g.q[k];
-                v = make_double2(pv.x + g.fx * d.x - g.fy * d.y - qv.x, pv.y + g.fx * d.y + g.fy * d.x - qv.y);
-            } else if (g.mode == 3) {
-                v = csub(g.out[k], v);
-            }
-            g.out[k] = v;
-        }
-}
 
 // ---- density: part[s][r] = sum over this split's orbitals of |psi_i(r)|^2; rho = sum_s part (fixed order) -----------------
 __global__ void __launch_bounds__(256) density_partial(const cd *psi, long long n_pts, int n, int per_split, double *part) {
