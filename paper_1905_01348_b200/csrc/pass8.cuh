@@ -25,36 +25,40 @@
 
 namespace ptfock {
 
-template <int N0_, int N1_, int N2_, int A1_, int A2_, int A0_>
+template <int N0_, int N1_, int N2_, int A1_, int A2_, int A0_, int MAXREG_A_ = 168, int MAXREG_C_ = 255, int NBUF_C_ = 3>
 struct P8 {
     static constexpr int N0 = N0_, N1 = N1_, N2 = N2_, A1 = A1_, A2 = A2_, A0 = A0_;
     static constexpr int B1 = N1 / A1, B2 = N2 / A2, B0 = N0 / A0;
     static_assert(A1 * B1 == N1 && A2 * B2 == N2 && A0 * B0 == N0, "bad split");
-    static_assert(B0 == 32 && A0 * B1 == 32, "pass B works on 32 x 32 points per slab position");
+    static_assert(B0 % 8 == 0 && B2 % 8 == 0, "the XOR swizzles work on groups of 8");
     static constexpr int RQ = 4, NQ = B1 / RQ;              // b1 = q*RQ + r
     static_assert(NQ * RQ == B1, "B1 must be a multiple of 4");
-    static constexpr int NT = RQ * B2;                      // slab passes: stage-1 tasks (r, b2)
-    static constexpr int NT2 = A1 * A2 * RQ;                // stage-2 tasks (k1a, k2a, r)
-    static_assert(NT == NT2 && NT == 64, "one task per thread in both stages");
+    // slab passes: stage-1 tasks (r, b2), A1*A2 points each; stage-2 tasks (k1a, k2a, r), B2 points each
+    static constexpr int NT1 = RQ * B2, NT2 = A1 * A2 * RQ;
+    static constexpr int NT = ((NT1 > NT2 ? NT1 : NT2) + 31) / 32 * 32;
     static constexpr int QPTS = A1 * RQ * N2;               // points of one (slab, q) row of the scratch
+    static_assert(QPTS == NT1 * A1 * A2 && QPTS == NT2 * B2 && NT2 % 8 == 0, "task counts");
     static constexpr int NPOS = A1 * A2 * B2;               // slab positions (k2b, k1a, k2a) per row
     static constexpr int NBUF_A = 2;                        // pass A: ring of landed phi_i quarter slabs
     static constexpr int SMEM_A = NBUF_A * QPTS * 16 + 64;
-    static constexpr int NBUF_C = 3;                        // pass C: ring of landed pair-density rows
+    static constexpr int NBUF_C = NBUF_C_;                  // pass C: ring of landed pair-density rows
     static constexpr int SMEM_C = NBUF_C * QPTS * 16 + 64;
-    static constexpr int MAXREG_A = 168, MAXREG_C = 255;    // 6 / 4 CTAs per SM
-    // pass B
+    static constexpr int MAXREG_A = MAXREG_A_, MAXREG_C = MAXREG_C_;
+    // pass B: tile = [q][x0][P positions x RQ r] (128-byte rows); stage-1 / 3 tasks (b0, p): the A0 x B1 points
+    // (a0, b1) at x0 = a0*B0 + b0; middle tasks (k0a, k1b, p): the B0 points b0
     static constexpr int P = 2;                             // slab positions per tile: rows of P*RQ*16 = 128 bytes
     static constexpr int ROWS = NQ * N0;                    // tile rows (q, x0)
-    static_assert(ROWS <= 256, "TMA box limit");
-    static constexpr int TILE_B = ROWS * P * RQ * 16;       // 32 KB
-    static constexpr int NTB = 32 * P;                      // 64 threads
-    static_assert(A0 * NQ * P * RQ == NTB, "middle-stage tasks");
-    static constexpr int GB = 3;                            // tiles (64-thread groups) per CTA, sharing one copy of v'
-    static constexpr int V_BYTES = ROWS * P * RQ * 8;       // 16 KB
-    static constexpr int SMEM_B = GB * TILE_B + V_BYTES + 64;   // + mbarriers: 2 CTAs (6 tiles) per SM
-    static constexpr int MAXREG_B = 168;                    // 12 warps per SM
+    static_assert(ROWS <= 256 && ROWS % 8 == 0, "TMA box limit; 1 KB swizzle period");
+    static constexpr int TILE_B = ROWS * P * RQ * 16;
+    static constexpr int NTB1 = B0 * P, NTB2 = A0 * B1 * P;
+    static constexpr int NTB = ((NTB1 > NTB2 ? NTB1 : NTB2) + 31) / 32 * 32;    // threads of one tile's group
+    static_assert(NTB1 * A0 * B1 == ROWS * P * RQ && NTB2 * B0 == ROWS * P * RQ, "pass B task counts");
+    static constexpr int GB = 3;                            // tiles (groups) per CTA, sharing one copy of v'
+    static constexpr int V_BYTES = ROWS * P * RQ * 8;       // = NTB2 * B0 doubles
+    static constexpr int SMEM_B = GB * TILE_B + V_BYTES + 64;   // + mbarriers
+    static constexpr int MAXREG_B = 168;
     static constexpr int NGRP = NPOS / P;                   // tiles per pair
+    static_assert(NPOS % P == 0, "positions per tile");
 };
 
 // ---- DFT32 = 4 x 8 (register resident, natural order in and out) -----------------------------------------------
@@ -152,6 +156,7 @@ template <class S>
 __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ;
     constexpr int NBUF = S::NBUF_A, CH = RQ * N2;        // one a1 chunk: RQ contiguous rows
+    constexpr bool ALL1 = S::NT1 == S::NT, ALL2 = S::NT2 == S::NT;     // every thread owns a stage-1 / stage-2 task
     extern __shared__ __align__(128) unsigned char smem_raw[];
     cd *ring = reinterpret_cast<cd *>(smem_raw);
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
@@ -162,8 +167,10 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     tri_range(g.tri, jj, blockIdx.z * per, min(g.na, blockIdx.z * per + per), ii_beg, ii_end);
     const int n_it = ii_end - ii_beg;
     if (n_it <= 0) return;
-    // stage-1 task (r, b2): the 4 x 4 points (a1, a2) at x1 = a1*B1 + b1, x2 = a2*B2 + b2
-    const int b2 = tid % B2, r = tid / B2, b1 = q * RQ + r;
+    // stage-1 task (r, b2): the A1 x A2 points (a1, a2) at x1 = a1*B1 + b1, x2 = a2*B2 + b2
+    const bool act1 = ALL1 || tid < S::NT1, act2 = ALL2 || tid < S::NT2;
+    const int t1 = act1 ? tid : 0;
+    const int b2 = t1 % B2, r = t1 / B2, b1 = q * RQ + r;
     const long long off1 = (long long)x0 * (N1 * N2) + b1 * N2 + b2;
     // chunk a1 of the quarter slab of orbital it: phi0 + it*grid_pts + a1*B1*N2
     const cd *phi0 = g.a + (long long)(g.a0 + ii_beg) * g.grid_pts + (long long)x0 * (N1 * N2) + (q * RQ) * N2;
@@ -187,7 +194,7 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
             if (k < n_it) issue(k);
     }
     cd pj[A1 * A2];
-    {
+    if (act1) {
         const cd *psi = g.b + (long long)(g.b0 + jj) * g.grid_pts + off1;
 #pragma unroll
         for (int a1 = 0; a1 < A1; ++a1)
@@ -201,43 +208,49 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     for (int k = 1; k < A2; ++k) tw2[k - 1] = g.tw2[b2 * k];          // w_N2^(b2 k2a)
     const int ld1 = r * N2 + b2;                                       // + a1*CH + a2*B2
     const long long pair0 = (long long)ii_beg * g.stride_loop + (long long)jj * g.stride_cta;
-    cd *dst = g.scratch + ((pair0 * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS + tid;
+    cd *dst = g.scratch + ((pair0 * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS + (act2 ? tid : 0);
     const long long dst_step = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
 #pragma unroll 1
     for (int it = 0; it < n_it; ++it) {
         cd *T = ring + (it % NBUF) * S::QPTS;
         mbar_wait(&bars[it % NBUF], (it / NBUF) & 1);
         cd u[A1 * A2];
+        if (act1) {
 #pragma unroll
-        for (int a1 = 0; a1 < A1; ++a1)
+            for (int a1 = 0; a1 < A1; ++a1)
 #pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) u[a1 * A2 + a2] = T[ld1 + a1 * CH + a2 * B2];
+                for (int a2 = 0; a2 < A2; ++a2) u[a1 * A2 + a2] = T[ld1 + a1 * CH + a2 * B2];
+        }
         fence_proxy_async();
         __syncthreads();                                // phi_i read; the buffer of iteration it - 1 is free
         if (tid < 32 && it + NBUF - 1 < n_it) issue(it + NBUF - 1);
+        if (act1) {
 #pragma unroll
-        for (int k = 0; k < A1 * A2; ++k) u[k] = cmulc(pj[k], u[k]);  // psi_j conj(phi_i)
-        dft_rows<A1, A2, false>(u);
+            for (int k = 0; k < A1 * A2; ++k) u[k] = cmulc(pj[k], u[k]);  // psi_j conj(phi_i)
+            dft_rows<A1, A2, false>(u);
 #pragma unroll
-        for (int k1 = 1; k1 < A1; ++k1)
+            for (int k1 = 1; k1 < A1; ++k1)
 #pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) u[k1 * A2 + a2] = cmul(u[k1 * A2 + a2], tw1[k1 - 1]);
-        dft_cols<A1, A2, false>(u);
+                for (int a2 = 0; a2 < A2; ++a2) u[k1 * A2 + a2] = cmul(u[k1 * A2 + a2], tw1[k1 - 1]);
+            dft_cols<A1, A2, false>(u);
 #pragma unroll
-        for (int k2 = 1; k2 < A2; ++k2)
+            for (int k2 = 1; k2 < A2; ++k2)
 #pragma unroll
-            for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmul(u[k1 * A2 + k2], tw2[k2 - 1]);
-        // value (k1a, k2a) of this thread belongs to stage-2 task t2 = (k1a*A2 + k2a)*RQ + r, index b2
+                for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmul(u[k1 * A2 + k2], tw2[k2 - 1]);
+            // value (k1a, k2a) of this thread belongs to stage-2 task t2 = (k1a*A2 + k2a)*RQ + r, index b2
 #pragma unroll
-        for (int k = 0; k < A1 * A2; ++k) T[(k * RQ + r) * B2 + (b2 ^ ((k * RQ + r) & 7))] = u[k];
+            for (int k = 0; k < A1 * A2; ++k) T[(k * RQ + r) * B2 + (b2 ^ ((k * RQ + r) & 7))] = u[k];
+        }
         __syncthreads();
         // stage 2: task tid, DFT over b2; output k2b at k2b*NT2 + tid of the scratch row
-        cd w[B2];
+        if (act2) {
+            cd w[B2];
 #pragma unroll
-        for (int b = 0; b < B2; ++b) w[b] = T[tid * B2 + (b ^ (tid & 7))];
-        DFT<B2, false>::run(w);
+            for (int b = 0; b < B2; ++b) w[b] = T[tid * B2 + (b ^ (tid & 7))];
+            DFT<B2, false>::run(w);
 #pragma unroll
-        for (int m = 0; m < B2; ++m) dst[m * S::NT2] = w[m];
+            for (int m = 0; m < B2; ++m) dst[m * S::NT2] = w[m];
+        }
         dst += dst_step;
     }
 }
@@ -253,6 +266,7 @@ template <class S>
 __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ;
     constexpr int NBUF = S::NBUF_C, NT2 = S::NT2;
+    constexpr bool ALL1 = S::NT1 == S::NT, ALL2 = S::NT2 == S::NT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     cd *ring = reinterpret_cast<cd *>(smem_raw);
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
@@ -262,7 +276,9 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     tri_range(g.tri, tt, 0, g.na, it_lo, it_hi);
     const int n_it = it_hi - it_lo;
     if (n_it <= 0) return;
-    const int b2 = tid % B2, r = tid / B2, b1 = q * RQ + r;
+    const bool act1 = ALL1 || tid < S::NT1, act2 = ALL2 || tid < S::NT2;    // owner of a last-stage / first-stage task
+    const int t1 = act1 ? tid : 0;
+    const int b2 = t1 % B2, r = t1 / B2, b1 = q * RQ + r;
     const long long off1 = (long long)x0 * (N1 * N2) + b1 * N2 + b2;
     const long long pair_stride = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
     const cd *src = g.scratch + (((long long)tt * g.stride_cta * S::NQ + q) * S::N0 + x0) * (long long)S::QPTS
@@ -289,10 +305,12 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     for (int k = 0; k < A1 * A2; ++k) acc[k] = make_double2(0.0, 0.0);
     const cd *phi = g.a + (long long)(g.a0 + it_lo) * g.grid_pts + off1;
     cd f[A1 * A2];
+    if (act1) {
 #pragma unroll
-    for (int a1 = 0; a1 < A1; ++a1)
+        for (int a1 = 0; a1 < A1; ++a1)
 #pragma unroll
-        for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
+            for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
+    }
     const bool cw = g.conj_w != 0;
     __syncthreads();                                    // mbarrier inits visible
 #pragma unroll 1
@@ -300,8 +318,10 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
         cd *T = ring + (it % NBUF) * S::QPTS;
         mbar_wait(&bars[it % NBUF], (it / NBUF) & 1);
         cd w[B2];
+        if (act2) {
 #pragma unroll
-        for (int m = 0; m < B2; ++m) w[m] = T[m * NT2 + tid];
+            for (int m = 0; m < B2; ++m) w[m] = T[m * NT2 + tid];
+        }
         fence_proxy_async();
         __syncthreads();                                // row read; the buffer of iteration it - 1 is free
         if (tid == 0 && it + NBUF - 1 < n_it) {
@@ -310,44 +330,49 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
             bulk_g2s(ring + (nx % NBUF) * S::QPTS, src + (long long)nx * pair_stride, S::QPTS * 16u, &bars[nx % NBUF]);
         }
         // stage 1': inverse DFT over k2b of task tid = (k1a*A2 + k2a)*RQ + r, back in place (swizzled)
-        DFT<B2, true>::run(w);
+        if (act2) {
+            DFT<B2, true>::run(w);
 #pragma unroll
-        for (int b = 0; b < B2; ++b) T[b * NT2 + (tid ^ (b & 7))] = w[b];
-        __syncthreads();
-        cd u[A1 * A2];
-#pragma unroll
-        for (int k = 0; k < A1 * A2; ++k) u[k] = T[b2 * NT2 + ((k * RQ + r) ^ (b2 & 7))];
-#pragma unroll
-        for (int k2 = 1; k2 < A2; ++k2)
-#pragma unroll
-            for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmulc(u[k1 * A2 + k2], tw2[k2 - 1]);
-        dft_cols<A1, A2, true>(u);
-#pragma unroll
-        for (int k1 = 1; k1 < A1; ++k1)
-#pragma unroll
-            for (int a2 = 0; a2 < A2; ++a2) u[k1 * A2 + a2] = cmulc(u[k1 * A2 + a2], tw1[k1 - 1]);
-        dft_rows<A1, A2, true>(u);
-        if (cw) {
-#pragma unroll
-            for (int k = 0; k < A1 * A2; ++k) {
-                const cd pr = cmulc(f[k], u[k]);
-                acc[k].x += pr.x; acc[k].y += pr.y;
-            }
-        } else {
-#pragma unroll
-            for (int k = 0; k < A1 * A2; ++k) {
-                const cd pr = cmul(f[k], u[k]);
-                acc[k].x += pr.x; acc[k].y += pr.y;
-            }
+            for (int b = 0; b < B2; ++b) T[b * NT2 + (tid ^ (b & 7))] = w[b];
         }
-        phi += g.grid_pts;
-        if (it + 1 < n_it) {                            // next phi_i: on its way during the next iteration's first half
+        __syncthreads();
+        if (act1) {
+            cd u[A1 * A2];
 #pragma unroll
-            for (int a1 = 0; a1 < A1; ++a1)
+            for (int k = 0; k < A1 * A2; ++k) u[k] = T[b2 * NT2 + ((k * RQ + r) ^ (b2 & 7))];
 #pragma unroll
-                for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
+            for (int k2 = 1; k2 < A2; ++k2)
+#pragma unroll
+                for (int k1 = 0; k1 < A1; ++k1) u[k1 * A2 + k2] = cmulc(u[k1 * A2 + k2], tw2[k2 - 1]);
+            dft_cols<A1, A2, true>(u);
+#pragma unroll
+            for (int k1 = 1; k1 < A1; ++k1)
+#pragma unroll
+                for (int a2 = 0; a2 < A2; ++a2) u[k1 * A2 + a2] = cmulc(u[k1 * A2 + a2], tw1[k1 - 1]);
+            dft_rows<A1, A2, true>(u);
+            if (cw) {
+#pragma unroll
+                for (int k = 0; k < A1 * A2; ++k) {
+                    const cd pr = cmulc(f[k], u[k]);
+                    acc[k].x += pr.x; acc[k].y += pr.y;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < A1 * A2; ++k) {
+                    const cd pr = cmul(f[k], u[k]);
+                    acc[k].x += pr.x; acc[k].y += pr.y;
+                }
+            }
+            phi += g.grid_pts;
+            if (it + 1 < n_it) {                        // next phi_i: on its way during the next iteration's first half
+#pragma unroll
+                for (int a1 = 0; a1 < A1; ++a1)
+#pragma unroll
+                    for (int a2 = 0; a2 < A2; ++a2) f[a1 * A2 + a2] = ldcg_v(phi + a1 * (B1 * N2) + a2 * B2);
+            }
         }
     }
+    if (!act1) return;
     cd *o = g.out + (long long)(g.b0 + tt) * g.grid_pts + off1;
 #pragma unroll
     for (int a1 = 0; a1 < A1; ++a1)
@@ -362,7 +387,7 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
 
 // ---- pass B ---------------------------------------------------------------------------------------------------
 struct P8MidArgs {
-    const double2 *v;    // [tile group][16][64 threads]: the middle-stage thread's v' values (k0b = 2m, 2m + 1)
+    const double2 *v;    // [tile group][B0 / 2][NTB2 middle tasks]: the middle-stage thread's v' values (k0b = 2m, 2m + 1)
     const cd *tw0;       // exp(-2 pi i t / N0)
     int n_pairs;         // pairs in the wave
     int tri_nj;          // > 0: diagonal block of the symmetric schedule, pair = i*tri_nj + j exists only for i <= j
@@ -388,7 +413,7 @@ PTF_DEV void tensor_s2g_2d_sw(const CUtensorMap *map, int c0, int c1, const void
 // sits at (R*8 + (e ^ (R & 7))) * 16 bytes of the tile.
 template <class S>
 __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensorMap map, const P8MidArgs g) {
-    constexpr int N0 = S::N0, A0 = S::A0, B1 = S::B1, RQ = S::RQ, NQ = S::NQ, P = S::P, GB = S::GB;
+    constexpr int N0 = S::N0, A0 = S::A0, B0 = S::B0, B1 = S::B1, RQ = S::RQ, NQ = S::NQ, P = S::P, GB = S::GB;
     // the 128-byte swizzle pattern repeats every 1 KB: the tiles must start on 1 KB boundaries of the shared window
     extern __shared__ __align__(1024) unsigned char smem_b[];
     const double2 *vs = reinterpret_cast<const double2 *>(smem_b + GB * S::TILE_B);
@@ -413,24 +438,26 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
                 tensor_g2s_2d_sw(smem_b + k * S::TILE_B, &map, grp_pos * (P * RQ * 2), (g.pair0 + blockIdx.y * GB + k) * S::ROWS, &bars[k]);
             }
     }
-    // stage 1 / 3 task: (b0 = x0 mod 32, p); element (a0, q, r) at row q*N0 + a0*32 + b0, chunk (p*RQ + r) ^ (b0 & 7)
-    const int b0 = tid % 32, p = tid / 32;
+    // stage 1 / 3 task (b0, p): element (a0, q, r) at row q*N0 + a0*B0 + b0, chunk (p*RQ + r) ^ (b0 & 7)
+    const bool act1 = S::NTB1 == S::NTB || tid < S::NTB1, act2 = S::NTB2 == S::NTB || tid < S::NTB2;
+    const int t1 = act1 ? tid : 0, t2 = act2 ? tid : 0;
+    const int b0 = t1 % B0, p = t1 / B0;
     cd tw[A0 - 1];
 #pragma unroll
     for (int k = 1; k < A0; ++k) tw[k - 1] = g.tw0[b0 * k];           // w_N0^(b0 k0a)
-    // middle task: tid = ((k0a*NQ + q)*P + p)*RQ + r; element b0' at row q*N0 + k0a*32 + b0', chunk (p*RQ + r) ^ (b0' & 7)
-    const int mr = tid % RQ, mp = (tid / RQ) % P, mq = (tid / (RQ * P)) % NQ, mk = tid / (RQ * P * NQ);
-    const int rb = (mq * N0 + mk * 32) * 8, mc = mp * RQ + mr;
+    // middle task: t2 = ((k0a*NQ + q)*P + p)*RQ + r; element b0' at row q*N0 + k0a*B0 + b0', chunk (p*RQ + r) ^ (b0' & 7)
+    const int mr = t2 % RQ, mp = (t2 / RQ) % P, mq = (t2 / (RQ * P)) % NQ, mk = t2 / (RQ * P * NQ);
+    const int rb = (mq * N0 + mk * B0) * 8, mc = mp * RQ + mr;
     __syncthreads();                                    // mbarrier inits visible; from here on the groups are independent
     if (pair >= g.n_pairs || (g.tri_nj > 0 && pair / g.tri_nj > pair % g.tri_nj)) return;
-    auto group_sync = [&]() {                           // named barrier 1 + gi over the group's 64 threads
+    auto group_sync = [&]() {                           // named barrier 1 + gi over the group's threads
         if (gi == 0) asm volatile("bar.sync 1, %0;" ::"n"(S::NTB) : "memory");
         else if (gi == 1) asm volatile("bar.sync 2, %0;" ::"n"(S::NTB) : "memory");
         else asm volatile("bar.sync 3, %0;" ::"n"(S::NTB) : "memory");
     };
     static_assert(GB <= 3, "one named barrier per group");
     mbar_wait(&bars[gi], 0);
-    {
+    if (act1) {
         cd u[A0 * B1];                                                  // u[a0*B1 + b1], b1 = q*RQ + r
 #pragma unroll
         for (int a0 = 0; a0 < A0; ++a0)
@@ -438,7 +465,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
             for (int q = 0; q < NQ; ++q)
 #pragma unroll
                 for (int r = 0; r < RQ; ++r)
-                    u[a0 * B1 + q * RQ + r] = s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))];
+                    u[a0 * B1 + q * RQ + r] = s[(q * N0 + a0 * B0 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))];
         dft_rows<A0, B1, false>(u);
 #pragma unroll
         for (int k = 1; k < A0; ++k)
@@ -451,27 +478,27 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
             for (int q = 0; q < NQ; ++q)
 #pragma unroll
                 for (int r = 0; r < RQ; ++r)
-                    s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))] = u[a0 * B1 + q * RQ + r];
+                    s[(q * N0 + a0 * B0 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))] = u[a0 * B1 + q * RQ + r];
     }
     group_sync();
     mbar_wait(&bars[GB], 0);                            // v' landed (requested before the tiles)
-    {
-        cd u[32];
+    if (act2) {
+        cd u[B0];
 #pragma unroll
-        for (int b = 0; b < 32; ++b) u[b] = s[rb + b * 8 + (mc ^ (b & 7))];
-        DFT<32, false>::run(u);
+        for (int b = 0; b < B0; ++b) u[b] = s[rb + b * 8 + (mc ^ (b & 7))];
+        DFT<B0, false>::run(u);
 #pragma unroll
-        for (int m = 0; m < 16; ++m) {
-            const double2 vv = vs[m * S::NTB + tid];
+        for (int m = 0; m < B0 / 2; ++m) {
+            const double2 vv = vs[m * S::NTB2 + tid];
             u[2 * m] = cscale(u[2 * m], vv.x);
             u[2 * m + 1] = cscale(u[2 * m + 1], vv.y);
         }
-        DFT<32, true>::run(u);
+        DFT<B0, true>::run(u);
 #pragma unroll
-        for (int b = 0; b < 32; ++b) s[rb + b * 8 + (mc ^ (b & 7))] = u[b];
+        for (int b = 0; b < B0; ++b) s[rb + b * 8 + (mc ^ (b & 7))] = u[b];
     }
     group_sync();
-    {
+    if (act1) {
         cd u[A0 * B1];
 #pragma unroll
         for (int a0 = 0; a0 < A0; ++a0)
@@ -479,7 +506,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
             for (int q = 0; q < NQ; ++q)
 #pragma unroll
                 for (int r = 0; r < RQ; ++r)
-                    u[a0 * B1 + q * RQ + r] = s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))];
+                    u[a0 * B1 + q * RQ + r] = s[(q * N0 + a0 * B0 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))];
         dft_cols<A0, B1, true>(u);
 #pragma unroll
         for (int k = 1; k < A0; ++k)
@@ -492,7 +519,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
             for (int q = 0; q < NQ; ++q)
 #pragma unroll
                 for (int r = 0; r < RQ; ++r)
-                    s[(q * N0 + a0 * 32 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))] = u[a0 * B1 + q * RQ + r];
+                    s[(q * N0 + a0 * B0 + b0) * 8 + ((p * RQ + r) ^ (b0 & 7))] = u[a0 * B1 + q * RQ + r];
     }
     fence_proxy_async();
     group_sync();

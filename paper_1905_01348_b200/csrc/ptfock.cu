@@ -139,7 +139,7 @@ const PencilEntry kPencils[] = { PENCIL_REG(16), PENCIL_REG(32), PENCIL_REG(48),
 // ---- 8 + 10 + 8 bit split (pass8.cuh) ---------------------------------------------------------------------------
 struct P8Entry {
     int n0, n1, n2, a0, a1, a2;                 // k0 = k0a + a0*k0b, k1 = k1a + a1*k1b, k2 = k2a + a2*k2b
-    int nq, rq, p, rows, qpts, npos, ntb, minb_ac;
+    int nq, rq, p, rows, qpts, npos, ntb2, b0;    // ntb2 = middle-stage tasks of a pass B tile, b0 = their points
     void (*fwd)(const SlabArgs &, dim3, cudaStream_t);
     void (*inv)(const SlabArgs &, dim3, cudaStream_t);
     void (*mid)(const CUtensorMap &, const P8MidArgs &, int pairs, cudaStream_t);
@@ -160,10 +160,14 @@ template <class S> cudaError_t prepare_p8() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(p8_mid<S>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     return e;
 }
-typedef P8<64, 64, 64, 4, 4, 2> P8_64;
-#define P8E(S) { S::N0, S::N1, S::N2, S::A0, S::A1, S::A2, S::NQ, S::RQ, S::P, S::ROWS, S::QPTS, S::NPOS, S::NTB, 6, \
+//         N0  N1  N2  A1 A2 A0  regs A / C  ring C
+typedef P8<64, 64, 64, 4, 4, 2> P8_64;                     // 16-point stages: 64 threads, 6 / 4 CTAs per SM
+typedef P8<32, 32, 32, 4, 2, 2, 128, 200, 3> P8_32;        // 8-point first stage (4 x 2): 64 threads; pass B 2 x 8 | 16
+// (48^3 as P8<48, 48, 48, 6, 3, 3>, 18-point first stages at 224 / 255 registers and 12 KB pass B tiles, measured slower
+//  than the three-stage kernels: Si216 315 vs 246 ms, profiles/r02_rejected_variants.md; 48^3 stays on slabx / pencil_mid)
+#define P8E(S) { S::N0, S::N1, S::N2, S::A0, S::A1, S::A2, S::NQ, S::RQ, S::P, S::ROWS, S::QPTS, S::NPOS, S::NTB2, S::B0, \
                  launch_p8_fwd<S>, launch_p8_inv<S>, launch_p8_mid<S>, prepare_p8<S> }
-const P8Entry kP8[] = { P8E(P8_64) };
+const P8Entry kP8[] = { P8E(P8_64), P8E(P8_32) };
 #undef P8E
 
 // position -> frequency index of the digit-permuted order the forward passes leave an axis in
@@ -344,12 +348,12 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, b
         return PTFOCK_OK;
     }
     if (p8) {
-        // pass8.cuh order: [tile group][m < 16][middle-stage thread t < ntb] pairs (k0b = 2m, 2m + 1), where
+        // pass8.cuh order: [tile group][m < b0 / 2][middle-stage task t < ntb2] pairs (k0b = 2m, 2m + 1), where
         // t = ((k0a*nq + q)*p + pp)*rq + r, k1b = q*rq + r, slab position = group*p + pp = (k2b*a1 + k1a)*a2 + k2a
-        const int ngrp = p8->npos / p8->p;
+        const int ngrp = p8->npos / p8->p, hm = p8->b0 / 2;
         for (int grp = 0; grp < ngrp; ++grp)
-            for (int m = 0; m < 16; ++m)
-                for (int t = 0; t < p8->ntb; ++t) {
+            for (int m = 0; m < hm; ++m)
+                for (int t = 0; t < p8->ntb2; ++t) {
                     const int r = t % p8->rq, pp = (t / p8->rq) % p8->p, q = (t / (p8->rq * p8->p)) % p8->nq;
                     const int k0a = t / (p8->rq * p8->p * p8->nq);
                     const int pos = grp * p8->p + pp;
@@ -357,7 +361,7 @@ int build_vtable(const ptfock_desc &d, const SlabEntry &se, const P8Entry *p8, b
                     const int k1 = k1a + p8->a1 * (q * p8->rq + r), k2 = k2a + p8->a2 * k2b;
                     for (int h = 0; h < 2; ++h) {
                         const int k0 = k0a + p8->a0 * (2 * m + h);
-                        vperm[(((size_t)grp * 16 + m) * p8->ntb + t) * 2 + h] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
+                        vperm[(((size_t)grp * hm + m) * p8->ntb2 + t) * 2 + h] = scale * vnat[((size_t)k0 * n1 + k1) * n2 + k2];
                     }
                 }
         return PTFOCK_OK;

@@ -87,13 +87,15 @@ def test_Si64_full(cuda_device):
     assert _rel(out.cpu().numpy(), _oracle(cfg, phi)) <= TOL
 
 
-def test_schedules_agree(cuda_device):
-    """Symmetric schedule == general schedule on a copy of Phi == j-blocked calls; ragged tiles."""
+@pytest.mark.parametrize("flags", [0, binding.FLAG_THREE_STAGE_SLABS], ids=["two_stage", "three_stage"])
+def test_schedules_agree(cuda_device, flags):
+    """Symmetric schedule == general schedule on a copy of Phi == j-blocked calls; ragged tiles.  32^3: the two-stage
+    kernels (csrc/pass8.cuh) by default, the three-stage ones behind the flag."""
     cfg = synth.Config("s", (20.52,) * 3, (32, 32, 32), 13, synth.KERNEL_HSE)
     phi = synth.orbitals(cfg, device=cuda_device)
-    with binding.plan_for(cfg, block_i=4, block_j=4) as plan:
+    with binding.plan_for(cfg, block_i=4, block_j=4, flags=flags) as plan:
         sym = plan.apply(phi)
-        assert plan.info()["last_symmetric"] == 1
+        assert plan.info()["last_symmetric"] == 1 and plan.info()["pass8"] == (0 if flags else 1)
         gen = plan.apply(phi, phi.clone())
         assert plan.info()["last_symmetric"] == 0
         blk = torch.cat([plan.apply(phi, None, self_offset=o, n_targets=min(5, 13 - o)) for o in range(0, 13, 5)])

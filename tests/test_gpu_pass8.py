@@ -139,3 +139,47 @@ def test_wrong_device_pointer_is_rejected(cuda_device):
         rc = binding.lib().ptfock_apply(plan._h, ctypes.c_void_p(host.data_ptr()), None, 0, 2,
                                         ctypes.c_void_p(host.data_ptr()), None)
         assert rc == -1
+
+
+# ---- the same two-stage kernels instantiated for 32^3 (Si64: 4 x 2 | 16 slab stages, 2 x 8 | 16 pencil stages): thread
+# ---- counts differ between the stages (guards)
+@pytest.mark.parametrize("n", [32])
+def test_small_cubic_grids_general_and_symmetric(cuda_device, n):
+    edges = (10.26 * n / 16,) * 3
+    cfg = synth.Config("p8n", edges, (n, n, n), 7, synth.KERNEL_HSE, separate_psi=True)
+    phi = synth.random_orbitals(cfg, 31, 7, cuda_device)
+    psi = synth.random_orbitals(cfg, 32, 5, cuda_device)
+    outs = []
+    for flags in (0, binding.FLAG_THREE_STAGE_SLABS):
+        with binding.plan_for(cfg, max_targets=5, block_i=4, block_j=3, flags=flags) as plan:
+            outs.append(plan.apply(phi, psi))           # ragged i and j blocks, two waves in flight
+            torch.cuda.synchronize()
+            assert plan.info()["pass8"] == (0 if flags else 1)
+    ref = _oracle(cfg, phi, psi)
+    assert _rel(outs[0].cpu().numpy(), ref) <= TOL and _rel(outs[1].cpu().numpy(), ref) <= TOL
+    # symmetric schedule with triangular diagonal blocks and the conj(W) accumulate, bare Coulomb
+    cfg2 = synth.Config("p8ns", edges, (n, n, n), 6, synth.KERNEL_COULOMB)
+    with binding.plan_for(cfg2, block_i=2, block_j=2) as plan:
+        sym = plan.apply(phi[:6].contiguous())
+        again = plan.apply(phi[:6].contiguous())
+        torch.cuda.synchronize()
+        info = plan.info()
+    assert info["last_symmetric"] == 1 and info["last_pairs"] == 21 and info["pass8"] == 1
+    assert torch.equal(sym, again)
+    assert _rel(sym.cpu().numpy(), _oracle(cfg2, phi[:6])) <= TOL
+
+
+@pytest.mark.parametrize("n", [32])
+def test_small_cubic_grids_skew_cell(cuda_device, n):
+    """A skew cell: the v' table has no symmetry to lean on, every (k0, k1, k2) -> table slot must be right."""
+    a = 10.26 * n / 16
+    cell = [a, 0.0, 0.0, 0.21 * a, 0.93 * a, 0.0, 0.13 * a, -0.17 * a, 1.07 * a]
+    cfg = synth.Config("p8k", (a, a, a), (n, n, n), 2, synth.KERNEL_HSE)
+    phi = synth.random_orbitals(cfg, 33, 2, cuda_device)
+    psi = synth.random_orbitals(cfg, 34, 1, cuda_device)
+    with binding.Plan(cell, (n, n, n), 2, 1, synth.KERNEL_HSE, 0.106, 1.0) as plan:
+        out = plan.apply(phi, psi)
+        torch.cuda.synchronize()
+        assert plan.info()["pass8"] == 1
+    ref = oracle.apply(cell, (n, n, n), synth.KERNEL_HSE, 0.106, 1.0, phi.cpu().numpy(), psi.cpu().numpy(), None)
+    assert _rel(out.cpu().numpy(), ref) <= TOL

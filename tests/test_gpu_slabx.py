@@ -19,7 +19,7 @@ SHAPES = [
     ("s64x64", (11.0, 41.04, 41.04), (16, 64, 64)),        # kind P, bulk stores, three tiles
     ("s128x48", (11.0, 82.08, 30.78), (16, 128, 48)),      # kind Q, 24-point stage, two tiles
     ("s48x48", (11.0, 30.78, 30.78), (16, 48, 48)),        # kind Q, 9-point stage, 144-task DFT16 stages
-    ("s32x32", (11.0, 20.52, 20.52), (32, 32, 32)),        # kind Q, 4-point stage, 64-task DFT16 stages
+    ("s32x32", (11.0, 20.52, 20.52), (16, 32, 32)),        # kind Q, 4-point stage, 64-task DFT16 stages (32^3 itself: pass8)
     ("s90x60", (11.0, 61.56, 41.04), (16, 90, 60)),        # paper grid's slab: 24-point stage (6 x 4), DFT15 stages, 225 of 256 threads in stage 1
 ]
 
