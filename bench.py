@@ -17,6 +17,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import subprocess
@@ -382,6 +383,54 @@ def dense_leg(cfg, args, dev, local):
     print(json.dumps(line), flush=True)
 
 
+def ptcn_leg(cfg, args, dev, local):
+    """--leg ptcn: whole PT-CN time steps (Algorithm 1: residual, Anderson-mixed fixed point, density,
+    re-orthogonalisation) with the model Hamiltonian of DESIGN.md Q17 at cfg's grid and orbital count, sequenced over
+    the C ABI by paper_1905_01348_b200/ptcn.py; wall time per step (host least-squares included) and the share of it
+    spent applying the exchange operator."""
+    import torch
+    from paper_1905_01348_b200 import binding, ptcn, synth
+    n_e = cfg.n_occ
+    psi = synth.orbitals(cfg, cfg.seed_phi, n_e, dev)
+    x = torch.meshgrid(*[torch.arange(k, dtype=torch.float64) / k for k in cfg.n], indexing="ij")
+    v_ext = 0.2 * torch.cos(2 * math.pi * x[0]) + 0.1 * torch.sin(2 * math.pi * (x[1] + x[2]))
+    # a.u. (9.7 as).  The paper steps 50 as (PAPER.md:206) with its production solver; the plain Anderson-mixed fixed
+    # point of DESIGN.md Q18 has no preconditioner and converges for dt * (spectral width) / 2 up to ~10
+    dt = 0.4
+    steps_out = []
+    with ptcn.PTCN(cfg.cell, cfg.n, n_e, kernel=cfg.kernel, omega=cfg.omega, alpha=0.25, v_ext=v_ext, g=0.5, device=local) as st:
+        fock_ms = [0.0]
+        apply0 = st.fock.apply
+
+        def timed_apply(*a, **k):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            out = apply0(*a, **k)
+            e1.record()
+            fock_ms.append((e0, e1))
+            return out
+        st.fock.apply = timed_apply
+        for k in range(args.steps + 1):             # first step: warm-up
+            del fock_ms[:]
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            psi, info = st.step(psi, dt, tol=1e-8)
+            torch.cuda.synchronize()
+            wall = (time.perf_counter() - t0) * 1e3
+            fock = sum(a.elapsed_time(b) for a, b in fock_ms)
+            if k:
+                steps_out.append({"ms": wall, "fock_exchange_ms": fock, "fock_applications": len(fock_ms),
+                                  "scf_iterations": info["iterations"], "residual": info["residual"]})
+    ms = statistics.median(s["ms"] for s in steps_out)
+    line = {"metric": "PT-CN time step with a model Hamiltonian (fp64, 1 B200)", "unit": "ms per step", "value": ms,
+            "config": {"workload": f"{cfg.name}: {n_e} orbitals on {'x'.join(map(str, cfg.n))}, dt = {dt} a.u., "
+                                   "alpha = 0.25, residual < 1e-8", "leg": "ptcn"},
+            "dtype": "f64", "data": "synthetic", "steps": args.steps, "higher_is_better": False,
+            "fock_exchange_share": statistics.median(s["fock_exchange_ms"] / s["ms"] for s in steps_out),
+            "per_step": steps_out}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -399,9 +448,10 @@ def main():
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the second headline config (one Si1536 j-block) that the default Si512 run also times")
     ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")
-    ap.add_argument("--leg", default="fock", choices=["fock", "dense", "copybw"],
+    ap.add_argument("--leg", default="fock", choices=["fock", "dense", "copybw", "ptcn"],
                     help="fock: the headline exchange path (default); dense: the dense-algebra neighbours; copybw: device "
-                         "copy bandwidth vs working-set size (L2-resident vs HBM; profiles/r02_l2_resident.md); own JSON lines")
+                         "copy bandwidth vs working-set size (L2-resident vs HBM; profiles/r02_l2_resident.md); ptcn: whole PT-CN time "
+                         "steps with the model Hamiltonian (use --config Si64 / Si216); own JSON lines")
     args = ap.parse_args()
 
     from paper_1905_01348_b200 import synth
@@ -436,9 +486,9 @@ def main():
         if dist is not None:
             dist.destroy_process_group()
         return
-    if args.leg == "dense":
+    if args.leg in ("dense", "ptcn"):
         if rank == 0:
-            dense_leg(cfg, args, dev, local)
+            (dense_leg if args.leg == "dense" else ptcn_leg)(cfg, args, dev, local)
         if dist is not None:
             dist.destroy_process_group()
         return

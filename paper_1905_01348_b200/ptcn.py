@@ -57,7 +57,11 @@ class PTCN:
         psi_half = f.axpby(1.0, psi_n, -0.5j * dt, r_n)                 # line 2
         psi_f = psi_half.clone()
         rho = f.density(psi_f)                                          # line 3
-        xs, rs = [], []
+        # Anderson history: differences of consecutive iterates / residuals (newest first) and their Gram matrix per
+        # wavefunction, grown by one row per iteration (the oldest difference drops out beyond `depth`)
+        x_prev = r_prev = None
+        dxs, drs = [], []
+        gram = np.zeros((n_e, 0, 0), dtype=np.complex128)
         info = {"iterations": 0, "rho_change": None, "residual": None}
         for it in range(max_iter):                                      # lines 4-10
             h = self.h_apply(psi_f)                                     # line 5
@@ -65,23 +69,26 @@ class PTCN:
             info["residual"] = float(np.sqrt(f.banddot(r_f, r_f).real.sum() / n_e))
             if info["residual"] < tol:
                 break
-            xs.append(psi_f)
-            rs.append(r_f)
-            if len(xs) > depth + 1:
-                xs.pop(0)
-                rs.pop(0)
-            m = len(xs) - 1
+            if x_prev is not None:
+                dxs.insert(0, f.axpby(1.0, psi_f, -1.0, x_prev))
+                drs.insert(0, f.axpby(1.0, r_f, -1.0, r_prev))
+                row = np.stack([f.banddot(drs[0], d) for d in drs], axis=1)        # <dR_new, dR_b> for every stored b
+                m_old = gram.shape[1]
+                g2 = np.empty((n_e, m_old + 1, m_old + 1), dtype=np.complex128)
+                g2[:, 1:, 1:] = gram
+                g2[:, 0, :] = row
+                g2[:, :, 0] = row.conj()
+                g2[:, 0, 0] = row[:, 0].real
+                gram = g2
+                if len(dxs) > depth:
+                    dxs.pop()
+                    drs.pop()
+                    gram = gram[:, :depth, :depth]
+            x_prev, r_prev = psi_f, r_f
+            m = len(dxs)
             new = f.axpby(1.0, psi_f, -beta, r_f)                       # line 7: Anderson mixing, per wavefunction
             if m > 0:
-                dxs = [f.axpby(1.0, xs[m - a], -1.0, xs[m - a - 1]) for a in range(m)]
-                drs = [f.axpby(1.0, rs[m - a], -1.0, rs[m - a - 1]) for a in range(m)]
-                gram = np.empty((n_e, m, m), dtype=np.complex128)
-                rhs = np.empty((n_e, m), dtype=np.complex128)
-                for a in range(m):
-                    rhs[:, a] = f.banddot(drs[a], r_f)
-                    for b in range(a, m):
-                        gram[:, a, b] = f.banddot(drs[a], drs[b])
-                        gram[:, b, a] = gram[:, a, b].conj()
+                rhs = np.stack([f.banddot(d, r_f) for d in drs], axis=1)
                 gamma = np.empty((n_e, m), dtype=np.complex128)
                 for j in range(n_e):
                     gj = gram[j] + 1e-14 * np.trace(gram[j]).real / m * np.eye(m)
