@@ -17,7 +17,7 @@
  * i.e. one grid = 16 N bytes, orbital k starts at byte 16 N k.  All orbital pointers must be
  * 16-byte aligned.  Unless a function says HOST, pointers are DEVICE pointers on the plan's device.
  *
- * Everything runs in hand-written sm_100a kernels; there is no CPU fallback: on a machine without
+ * Everything runs in hand-written sm_100a kernels (no cuFFT / cuBLAS / cuSOLVER); there is no CPU fallback: on a machine without
  * such a device ptfock_create returns PTFOCK_ERR_UNSUPPORTED_DEVICE (or PTFOCK_ERR_CUDA).
  *
  * Error behaviour: every function returns 0 (PTFOCK_OK) or a negative code below; nothing throws
@@ -30,8 +30,9 @@
  *   (64,64) (128,48) (48,48) (32,32) (90,60)            -- TMA-fed three-stage slab passes
  *   (16,16) (16,32) (32,16) (16,48) (48,32) (32,64)     -- generic slab passes
  * (all BASELINE.json configs, and the paper's own 60 x 90 x 120 grid stored as 120 x 90 x 60).
- * 64 x 64 x 64 additionally has the two-stage slab passes + 32 x 32 pencil pass, and 16 x 16 x 16 the single-pass
- * on-chip kernel (whole pair-solve in one CTA, no scratch); both are the default for their grid.
+ * 64 x 64 x 64 and 32 x 32 x 32 additionally have the two-stage slab passes + two-stage pencil pass, and 16 x 16 x 16
+ * the single-pass on-chip kernel (whole pair-solve in one CTA, no scratch); these are the default for their grids.
+ * The dense-algebra contractions (ptfock_overlap / rotate / residual / orthonormalize) run on the FP64 tensor cores.
  */
 #ifndef PTFOCK_H
 #define PTFOCK_H
