@@ -1,23 +1,27 @@
-// pass8.cuh -- the "8 + 10 + 8 bit" split of the pair-solve for 64^3 grids (Alg. 2 lines 6-10, Eq. (3)).
+// pass8.cuh -- the two-stage split of the pair-solve ("8 + 10 + 8 bits" at 64^3; Alg. 2 lines 6-10, Eq. (3)).
 //
-// The three passes of kernels.cuh / slabx.cuh give the slab passes 12 index bits (three butterfly stages, six
-// shared-memory crossings per point) and the pencil pass 6; ncu showed the slab passes bound by the L1/shared-memory
-// data pipe, not by HBM (profiles/r01_ncu_full_si512.md).  Here the slab passes keep only TWO stages and hand the low
-// digit b1 of x1 to the pencil pass, which has the slack:
+// The three passes of kernels.cuh / slabx.cuh give the slab passes three butterfly stages (six shared-memory crossings
+// per point) and the pencil pass one or two; ncu showed the slab passes bound by the L1 / shared-memory data pipe, not
+// by HBM (profiles/r01_ncu_full_si512.md).  Here the slab passes keep only TWO stages and hand the low digit b1 of x1
+// to the pencil pass, which has the slack:
 //
-//   x1 = a1*B1 + b1,  x2 = a2*B2 + b2          (64^3: A1 = 4, B1 = 16, A2 = 4, B2 = 16)
+//   x0 = a0*B0 + b0,  x1 = a1*B1 + b1,  x2 = a2*B2 + b2,  b1 = q*RQ + r  (RQ = 4)
 //   pass A  p8_fwd     : rho = conj(phi_i) psi_j;  2-D DFT over (a1, a2) + both twiddles | DFT over b2
-//                        one CTA = 64 threads = one (target, x0, quarter q of b1 = 4q + r); phi_i comes straight from
-//                        global memory into registers (128-bit, 256-byte runs), one padded exchange through shared
-//                        memory, results leave from registers in 1 KB runs: 4 crossings of the LSU pipe per point.
-//   pass B  p8_mid     : 2-D DFT over (x0, b1) = 64 x 16 = 32 x 32 points per slab position, x v'(G), inverse;
-//                        tile = [q][x0][2 positions x 4 r] (32 KB) by ONE swizzled tensor-map TMA load / store.
+//                        one CTA = one (target, x0, q); phi_i's rows (A1 runs of RQ*N2 elements) arrive by bulk async
+//                        copies (TMA) in a ring of shared-memory buffers, both stages work in place in the landed
+//                        buffer through an XOR swizzle, results leave from registers in runs of NT2 elements.
+//   pass B  p8_mid     : 2-D DFT over (x0, b1): stage (a0, b1) + twiddle | DFT over b0, x v'(G), and back;
+//                        tile = [q][x0][P positions x RQ r] (128-byte rows) by ONE swizzled tensor-map TMA load / store.
 //   pass C  p8_inv_acc : mirror of A; x phi_i and the sum over i in registers.
 //
-// Pair scratch: [pair][q][x0][k2b][k1a][k2a][r] (16-byte elements): a pass A / C CTA owns one contiguous 16 KB
-// row (pair, q, x0); pass B sees 256 rows (q, x0) of one pair, 128 contiguous bytes of each.
+// Instantiated for 64^3 (A1 = A2 = 4, A0 = 2: 16-point slab stages, 32 x 32 pencil stages; 64-thread CTAs / groups) and
+// 32^3 (A1 = 4, A2 = 2, A0 = 2: 8 | 16 and 16 | 16).  The stages' task counts may differ (NT1 != NT2, NTB1 != NTB2):
+// threads without a task only keep the barriers.
+//
+// Pair scratch: [pair][q][x0][k2b][k1a][k2a][r] (16-byte elements): a pass A / C CTA owns one contiguous row
+// (pair, q, x0) of QPTS elements; pass B sees the NQ*N0 rows (q, x0) of one pair, 128 contiguous bytes of each.
 // Frequencies: k0 = k0a + A0*k0b, k1 = k1a + A1*k1b, k2 = k2a + A2*k2b; nothing is ever un-permuted (the v' table is
-// stored in pass B's register order, build_vtable8).
+// stored in pass B's register order, build_vtable).
 #pragma once
 #include <cuda.h>
 #include "kernels.cuh"
