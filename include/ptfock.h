@@ -30,7 +30,7 @@
  *   (64,64) (128,48) (48,48) (32,32) (90,60)            -- TMA-fed three-stage slab passes
  *   (16,16) (16,32) (32,16) (16,48) (48,32) (32,64)     -- generic slab passes
  * (all BASELINE.json configs, and the paper's own 60 x 90 x 120 grid stored as 120 x 90 x 60).
- * 64 x 64 x 64 and 32 x 32 x 32 additionally have the two-stage slab passes + two-stage pencil pass, and 16 x 16 x 16
+ * 64 x 64 x 64, 48 x 48 x 48 and 32 x 32 x 32 additionally have the two-stage slab passes + two-stage pencil pass, and 16 x 16 x 16
  * the single-pass on-chip kernel (whole pair-solve in one CTA, no scratch); these are the default for their grids.
  * The dense-algebra contractions (ptfock_overlap / rotate / residual / orthonormalize) run on the FP64 tensor cores.
  */

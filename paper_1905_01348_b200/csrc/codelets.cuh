@@ -123,6 +123,9 @@ template <bool INV> struct DFT<15, INV> {
     }
 };
 
+// radix 24 = 3 x 8 by the same map: n = 8 n1 + 3 n2 (n1 < 3, n2 < 8); k = 16 k1 + 9 k2 mod 24.
+// (Declared after DFT<8>: see below.)
+
 template <bool INV> struct DFT<4, INV> {
     static PTF_DEV void run(cd &a0, cd &a1, cd &a2, cd &a3) {
         cd t0 = cadd(a0, a2), t1 = csub(a0, a2);
@@ -152,6 +155,25 @@ template <bool INV> struct DFT<8, INV> {
         v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
         v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
         v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
+    }
+};
+
+template <bool INV> struct DFT<24, INV> {
+    static PTF_DEV void run(cd (&v)[24]) {
+        cd a[3][8];
+#pragma unroll
+        for (int n1 = 0; n1 < 3; ++n1)
+#pragma unroll
+            for (int n2 = 0; n2 < 8; ++n2) a[n1][n2] = v[(8 * n1 + 3 * n2) % 24];
+#pragma unroll
+        for (int n1 = 0; n1 < 3; ++n1) DFT<8, INV>::run(a[n1]);
+#pragma unroll
+        for (int k2 = 0; k2 < 8; ++k2) {
+            cd c[3] = { a[0][k2], a[1][k2], a[2][k2] };
+            DFT<3, INV>::run(c);
+#pragma unroll
+            for (int k1 = 0; k1 < 3; ++k1) v[(16 * k1 + 9 * k2) % 24] = c[k1];
+        }
     }
 };
 

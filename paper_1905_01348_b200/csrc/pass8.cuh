@@ -14,8 +14,8 @@
 //                        tile = [q][x0][P positions x RQ r] (128-byte rows) by ONE swizzled tensor-map TMA load / store.
 //   pass C  p8_inv_acc : mirror of A; x phi_i and the sum over i in registers.
 //
-// Instantiated for 64^3 (A1 = A2 = 4, A0 = 2: 16-point slab stages, 32 x 32 pencil stages; 64-thread CTAs / groups) and
-// 32^3 (A1 = 4, A2 = 2, A0 = 2: 8 | 16 and 16 | 16).  The stages' task counts may differ (NT1 != NT2, NTB1 != NTB2):
+// Instantiated for 64^3 (A1 = A2 = 4, A0 = 2: 16-point slab stages, 32 x 32 pencil stages; 64-thread CTAs / groups),
+// 48^3 (A1 = A2 = 3, A0 = 2: 9 | 16 and 32 | 24) and 32^3 (A1 = 4, A2 = 2, A0 = 2: 8 | 16 and 16 | 16).  The stages' task counts may differ (NT1 != NT2, NTB1 != NTB2):
 // threads without a task only keep the barriers.
 //
 // Pair scratch: [pair][q][x0][k2b][k1a][k2a][r] (16-byte elements): a pass A / C CTA owns one contiguous row
@@ -41,12 +41,14 @@ struct P8 {
     static constexpr int NT1 = RQ * B2, NT2 = A1 * A2 * RQ;
     static constexpr int NT = ((NT1 > NT2 ? NT1 : NT2) + 31) / 32 * 32;
     static constexpr int QPTS = A1 * RQ * N2;               // points of one (slab, q) row of the scratch
-    static_assert(QPTS == NT1 * A1 * A2 && QPTS == NT2 * B2 && NT2 % 8 == 0, "task counts");
+    static_assert(QPTS == NT1 * A1 * A2 && QPTS == NT2 * B2, "task counts");
+    static constexpr int NT2P = (NT2 + 7) / 8 * 8;          // pass C's in-place exchange swizzles task indices in groups of 8
+    static constexpr int RING = B2 * NT2P;                  // elements of one ring buffer (>= QPTS)
     static constexpr int NPOS = A1 * A2 * B2;               // slab positions (k2b, k1a, k2a) per row
     static constexpr int NBUF_A = 2;                        // pass A: ring of landed phi_i quarter slabs
-    static constexpr int SMEM_A = NBUF_A * QPTS * 16 + 64;
+    static constexpr int SMEM_A = NBUF_A * RING * 16 + 64;
     static constexpr int NBUF_C = NBUF_C_;                  // pass C: ring of landed pair-density rows
-    static constexpr int SMEM_C = NBUF_C * QPTS * 16 + 64;
+    static constexpr int SMEM_C = NBUF_C * RING * 16 + 64;
     static constexpr int MAXREG_A = MAXREG_A_, MAXREG_C = MAXREG_C_;
     // pass B: tile = [q][x0][P positions x RQ r] (128-byte rows); stage-1 / 3 tasks (b0, p): the A0 x B1 points
     // (a0, b1) at x0 = a0*B0 + b0; middle tasks (k0a, k1b, p): the B0 points b0
@@ -163,7 +165,7 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     constexpr bool ALL1 = S::NT1 == S::NT, ALL2 = S::NT2 == S::NT;     // every thread owns a stage-1 / stage-2 task
     extern __shared__ __align__(128) unsigned char smem_raw[];
     cd *ring = reinterpret_cast<cd *>(smem_raw);
-    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::RING * 16);
     const int tid = threadIdx.x;
     const int jj = blockIdx.x, x0 = blockIdx.y / S::NQ, q = blockIdx.y % S::NQ;
     const int per = (g.na + gridDim.z - 1) / gridDim.z;
@@ -183,7 +185,7 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
         if (tid == 0) mbar_expect_tx(&bars[buf], S::QPTS * 16u);
         __syncwarp();
         if (tid < A1)
-            bulk_g2s(ring + buf * S::QPTS + tid * CH, phi0 + (long long)it * g.grid_pts + (long long)tid * (B1 * N2), CH * 16u, &bars[buf]);
+            bulk_g2s(ring + buf * S::RING + tid * CH, phi0 + (long long)it * g.grid_pts + (long long)tid * (B1 * N2), CH * 16u, &bars[buf]);
     };
     if (tid == 0) {
 #pragma unroll
@@ -216,7 +218,7 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
     const long long dst_step = (long long)g.stride_loop * S::NQ * S::N0 * S::QPTS;
 #pragma unroll 1
     for (int it = 0; it < n_it; ++it) {
-        cd *T = ring + (it % NBUF) * S::QPTS;
+        cd *T = ring + (it % NBUF) * S::RING;
         mbar_wait(&bars[it % NBUF], (it / NBUF) & 1);
         cd u[A1 * A2];
         if (act1) {
@@ -269,11 +271,11 @@ __global__ void __maxnreg__(S::MAXREG_A) p8_fwd(const SlabArgs g) {
 template <class S>
 __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     constexpr int N1 = S::N1, N2 = S::N2, A1 = S::A1, A2 = S::A2, B1 = S::B1, B2 = S::B2, RQ = S::RQ;
-    constexpr int NBUF = S::NBUF_C, NT2 = S::NT2;
+    constexpr int NBUF = S::NBUF_C, NT2 = S::NT2, NT2P = S::NT2P;
     constexpr bool ALL1 = S::NT1 == S::NT, ALL2 = S::NT2 == S::NT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     cd *ring = reinterpret_cast<cd *>(smem_raw);
-    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::QPTS * 16);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)NBUF * S::RING * 16);
     const int tid = threadIdx.x;
     const int tt = blockIdx.x, x0 = blockIdx.y / S::NQ, q = blockIdx.y % S::NQ;
     int it_lo, it_hi;
@@ -296,7 +298,7 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
         for (int k = 0; k < NBUF - 1; ++k)
             if (k < n_it) {
                 mbar_expect_tx(&bars[k], S::QPTS * 16u);
-                bulk_g2s(ring + k * S::QPTS, src + (long long)k * pair_stride, S::QPTS * 16u, &bars[k]);
+                bulk_g2s(ring + k * S::RING, src + (long long)k * pair_stride, S::QPTS * 16u, &bars[k]);
             }
     }
     cd tw1[A1 - 1], tw2[A2 - 1];
@@ -319,7 +321,7 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
     __syncthreads();                                    // mbarrier inits visible
 #pragma unroll 1
     for (int it = 0; it < n_it; ++it) {
-        cd *T = ring + (it % NBUF) * S::QPTS;
+        cd *T = ring + (it % NBUF) * S::RING;
         mbar_wait(&bars[it % NBUF], (it / NBUF) & 1);
         cd w[B2];
         if (act2) {
@@ -331,19 +333,19 @@ __global__ void __maxnreg__(S::MAXREG_C) p8_inv_acc(const SlabArgs g) {
         if (tid == 0 && it + NBUF - 1 < n_it) {
             const int nx = it + NBUF - 1;
             mbar_expect_tx(&bars[nx % NBUF], S::QPTS * 16u);
-            bulk_g2s(ring + (nx % NBUF) * S::QPTS, src + (long long)nx * pair_stride, S::QPTS * 16u, &bars[nx % NBUF]);
+            bulk_g2s(ring + (nx % NBUF) * S::RING, src + (long long)nx * pair_stride, S::QPTS * 16u, &bars[nx % NBUF]);
         }
         // stage 1': inverse DFT over k2b of task tid = (k1a*A2 + k2a)*RQ + r, back in place (swizzled)
         if (act2) {
             DFT<B2, true>::run(w);
 #pragma unroll
-            for (int b = 0; b < B2; ++b) T[b * NT2 + (tid ^ (b & 7))] = w[b];
+            for (int b = 0; b < B2; ++b) T[b * NT2P + (tid ^ (b & 7))] = w[b];      // pitch NT2P: the XOR stays in range
         }
         __syncthreads();
         if (act1) {
             cd u[A1 * A2];
 #pragma unroll
-            for (int k = 0; k < A1 * A2; ++k) u[k] = T[b2 * NT2 + ((k * RQ + r) ^ (b2 & 7))];
+            for (int k = 0; k < A1 * A2; ++k) u[k] = T[b2 * NT2P + ((k * RQ + r) ^ (b2 & 7))];
 #pragma unroll
             for (int k2 = 1; k2 < A2; ++k2)
 #pragma unroll

@@ -163,11 +163,12 @@ template <class S> cudaError_t prepare_p8() {
 //         N0  N1  N2  A1 A2 A0  regs A / C  ring C
 typedef P8<64, 64, 64, 4, 4, 2> P8_64;                     // 16-point stages: 64 threads, 6 / 4 CTAs per SM
 typedef P8<32, 32, 32, 4, 2, 2, 128, 200, 3> P8_32;        // 8-point first stage (4 x 2): 64 threads; pass B 2 x 8 | 16
+typedef P8<48, 48, 48, 3, 3, 2, 152, 232, 3> P8_48;        // 9-point first stage (3 x 3), DFT16; pass B 2 x 16 | DFT24 (x0 = 24 a0 + b0)
 // (48^3 as P8<48, 48, 48, 6, 3, 3>, 18-point first stages at 224 / 255 registers and 12 KB pass B tiles, measured slower
-//  than the three-stage kernels: Si216 315 vs 246 ms, profiles/r02_rejected_variants.md; 48^3 stays on slabx / pencil_mid)
+//  than the three-stage kernels: Si216 315 vs 246 ms, profiles/r02_rejected_variants.md #17)
 #define P8E(S) { S::N0, S::N1, S::N2, S::A0, S::A1, S::A2, S::NQ, S::RQ, S::P, S::ROWS, S::QPTS, S::NPOS, S::NTB2, S::B0, \
                  launch_p8_fwd<S>, launch_p8_inv<S>, launch_p8_mid<S>, prepare_p8<S> }
-const P8Entry kP8[] = { P8E(P8_64), P8E(P8_32) };
+const P8Entry kP8[] = { P8E(P8_64), P8E(P8_48), P8E(P8_32) };
 #undef P8E
 
 // position -> frequency index of the digit-permuted order the forward passes leave an axis in

@@ -143,7 +143,7 @@ def test_wrong_device_pointer_is_rejected(cuda_device):
 
 # ---- the same two-stage kernels instantiated for 32^3 (Si64: 4 x 2 | 16 slab stages, 2 x 8 | 16 pencil stages): thread
 # ---- counts differ between the stages (guards)
-@pytest.mark.parametrize("n", [32])
+@pytest.mark.parametrize("n", [32, 48])
 def test_small_cubic_grids_general_and_symmetric(cuda_device, n):
     edges = (10.26 * n / 16,) * 3
     cfg = synth.Config("p8n", edges, (n, n, n), 7, synth.KERNEL_HSE, separate_psi=True)
@@ -169,7 +169,7 @@ def test_small_cubic_grids_general_and_symmetric(cuda_device, n):
     assert _rel(sym.cpu().numpy(), _oracle(cfg2, phi[:6])) <= TOL
 
 
-@pytest.mark.parametrize("n", [32])
+@pytest.mark.parametrize("n", [32, 48])
 def test_small_cubic_grids_skew_cell(cuda_device, n):
     """A skew cell: the v' table has no symmetry to lean on, every (k0, k1, k2) -> table slot must be right."""
     a = 10.26 * n / 16
