@@ -164,6 +164,10 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
         harness.barrier(dev)
 
     n_i, n_j, wl = workload(cfg)
+    if args.full_application and cfg.j_block:
+        # the whole application V_X[Phi] Phi in one call: Phi AND out resident (2 x 38.65 GB at Si1536), pair-symmetric
+        # schedule over all block pairs (half the pair-solves of 32 streamed j-blocks)
+        n_j, wl = cfg.n_occ, f"{cfg.name}: whole application, {cfg.n_occ} targets x {cfg.n_occ} orbitals (Psi = Phi, symmetric schedule)"
     if args.targets:
         n_j = min(n_j, args.targets)
         wl += f" (slice: first {n_j} targets)"
@@ -174,7 +178,9 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
                             workspace_bytes=int(args.workspace_gb * (1 << 30)), flags=args.flags)
 
     def step():
-        if cfg.j_block or (args.targets and psi is None):
+        if args.full_application and cfg.j_block:
+            plan.apply(phi, out=out)
+        elif cfg.j_block or (args.targets and psi is None):
             plan.apply(phi, None, out=out, self_offset=0, n_targets=n_j)
         else:
             plan.apply(phi, psi, out=out)
@@ -226,6 +232,9 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
     # and writes it (v' amortised over the wave); C reads it, reads phi_i, and read-modify-writes out once per
     # (target, wave).  DESIGN.md 5.
     per_pair = [16.0 * N * (1.0 + 1.0 / Jb + 1.0 / Ib), 32.0 * N, 16.0 * N * (1.0 + 1.0 / Jb + 2.0 / Ib)]
+    if info1.get("last_symmetric"):
+        # pair-symmetric schedule: every executed pair density is read by two C launches (out_j, and out_i through conj)
+        per_pair[2] *= 2.0
     if info1.get("pass8") == 2:
         # on chip: phi_i twice (product, final multiply; the second read hits L1/L2), psi_j and the partial sums once per
         # CTA; no pair-density traffic at all.  Per pair-solve at most 32 N + (16 N + 32 N) / (orbitals per CTA).
@@ -310,7 +319,7 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
               "kernel": "HSE" if cfg.kernel == 1 else "Coulomb",
               "pair_solves_executed_per_step": pairs_exec, "symmetric_schedule": bool(info1["last_symmetric"]),
               "block_i": Ib, "block_j": Jb, "scratch_bytes": info1["scratch_bytes"],
-              "kernels": {0: "three-stage slab passes + pencil pass", 1: "pass8 (two-stage slab passes + 32x32 pencil pass)",
+              "kernels": {0: "three-stage slab passes + pencil pass", 1: "pass8 (two-stage slab passes + two-stage pencil pass)",
                           2: "onchip16 (whole pair-solve in one CTA, no scratch)"}[int(info1.get("pass8", 0))],
               "l2": f"inputs + scratch per step = {(16 * N * (n_i + 2 * n_j) + info1['scratch_bytes']) / 1e9:.2f} GB"
                     " (larger than the 126 MB L2; no explicit flush)",
@@ -445,6 +454,9 @@ def main():
     ap.add_argument("--targets", type=int, default=0, help="restrict the step to the first T targets (profiling slices)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--full-application", action="store_true",
+                    help="Si1536 / Si1536p: time the whole application (all 3072 targets, symmetric schedule, ~1 min per step) "
+                         "instead of one streamed j-block; use with --steps 1 --warmup 0 --no-e2e --no-cpu")
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the second headline config (one Si1536 j-block) that the default Si512 run also times")
     ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")

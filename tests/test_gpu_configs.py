@@ -87,6 +87,7 @@ def test_Si1536_streamed_j_blocks(cuda_device):
     with binding.plan_for(cfg) as plan:
         out = torch.empty((cfg.j_block,) + cfg.n, dtype=torch.complex128, device=cuda_device)
         # one tile-edge and one tile-interior column (J_b = 8) per block
+        refs = {}
         for offset, cols in ((0, [0, 43]), (1536, [50, 95])):
             plan.apply(phi, None, out=out, self_offset=offset, n_targets=cfg.j_block)
             torch.cuda.synchronize()
@@ -95,6 +96,18 @@ def test_Si1536_streamed_j_blocks(cuda_device):
             got = out[cols].cpu().numpy()
             err = float(np.abs(got - ref).max() / np.abs(ref).max())
             assert err <= TOL, (offset, err)
+            for k, c in enumerate(cols):
+                refs[offset + c] = ref[k]
+        # the whole application in ONE call (Phi and out both resident: 2 x 38.65 GB): the pair-symmetric schedule over
+        # all block pairs executes n (n + 1) / 2 pair-solves and must give the same columns
+        del out
+        full = plan.apply(phi)
+        torch.cuda.synchronize()
+        info = plan.info()
+        assert info["last_symmetric"] == 1 and info["last_pairs"] == 3072 * 3073 // 2
+        for c, ref in refs.items():
+            err = float(np.abs(full[c].cpu().numpy() - ref).max() / np.abs(ref).max())
+            assert err <= TOL, (c, err)
 
 
 def test_Si1536p_paper_grid_j_block(cuda_device):
