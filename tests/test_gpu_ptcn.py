@@ -81,3 +81,19 @@ def test_sharded_apply_world1_equals_apply(cuda_device):
             outs.append(plan.apply(phi, None, self_offset=lo, n_targets=hi - lo))
         torch.cuda.synchronize()
     assert torch.equal(torch.cat(outs), full)
+
+
+@pytest.mark.parametrize("n", [(32, 32, 32), (48, 48, 48), (64, 64, 64), (16, 32, 16)])
+def test_kinetic_plus_local_on_every_kernel_family(cuda_device, n):
+    """ptfock_hloc_apply runs the exchange passes with the constant orbital and the table |G|^2 / 2 (one 'orbital', a wave
+    of targets): on the two-stage kernels (32^3, 48^3, 64^3) and the generic three-stage ones, against the oracle's
+    plane-wave definition of the Laplacian (H Psi of Algorithm 1)."""
+    edges = (9.0 * n[0] / 16, 10.0 * n[1] / 16, 11.0 * n[2] / 16)
+    cell = [edges[0], 0, 0, 0, edges[1], 0, 0, 0, edges[2]]
+    cfg = synth.Config("kin", edges, n, 3, synth.KERNEL_HSE)
+    psi = synth.random_orbitals(cfg, 41, 3, cuda_device)
+    v = torch.rand(n, dtype=torch.float64, device=cuda_device)
+    with binding.Plan(cell, n, 1, 3, binding.KERNEL_KINETIC, 0.106, 1.0) as kin:
+        t = kin.hloc_apply(psi, v).cpu().numpy()
+    ref = ptcn_ref.kinetic_apply(cell, n, psi.cpu().numpy()) + v.cpu().numpy()[None] * psi.cpu().numpy()
+    assert np.abs(t - ref).max() <= 1e-12 * np.abs(ref).max()
