@@ -254,6 +254,7 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
     roofline = {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
                 # the path: SURVEY.md 8(d)'s contract roofline, 72 N bytes per executed pair-solve
                 "achieved": 72.0 * N * rate / 1e9, "frac": frac72, "survey_72N_frac": frac72,
+                "executed_pair_solves_per_s": rate,      # `value` is the EFFECTIVE rate n_i * n_j / time
                 "bytes_model": "72 N per executed pair-solve (SURVEY.md 8(d) B_3pass); own model below",
                 "own_bytes_per_pair_solve": sum(per_pair), "own_bytes_frac": rate / (peak * 1e9 / sum(per_pair)),
                 "worst_pass_frac": min(v["frac"] for v in per_kernel.values()),
