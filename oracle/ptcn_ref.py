@@ -18,8 +18,9 @@ Anderson mixing (reference [2] of the paper; fixed point of x -> x - R(x)), per 
     dX = [x_k - x_{k-1}, ..., x_{k-m+1} - x_{k-m}],  dR likewise.
 
 Pins: tests/test_oracle_ptcn_pins.py (stationary eigenstates, third-order agreement of the gauge-invariant density matrix
-with the exact propagator of a linear H, the converged Psi_f satisfies Eq. (5), orthonormal output, kinetic operator on
-plane waves).
+with the exact propagator of a linear H, the converged un-orthogonalised Psi_f satisfies Eq. (5) with H_f rebuilt from
+Psi_f to 1e-9, orthonormal output, kinetic operator on plane waves, H[Psi] against a dense matrix built point by point on
+4^3, the Anderson update solving per-wavefunction linear systems of dimension d in d + 1 iterations).
 """
 from __future__ import annotations
 
@@ -69,6 +70,26 @@ class Model:
         return np.ascontiguousarray(out)
 
 
+def anderson_update(xs, rs, beta: float, w: float = 1.0) -> np.ndarray:
+    """Line 7 of Algorithm 1: the next iterate from the stored iterates xs[0..m] and their residuals rs[0..m] (newest last),
+    one least-squares problem PER WAVEFUNCTION j (the formula is the module header's):
+        gamma_j = argmin || r_m[j] - dR_j gamma ||,   x_new[j] = x_m[j] - beta r_m[j] - (dX_j - beta dR_j) gamma_j.
+    xs[k], rs[k]: arrays [n_e, ...]; w: weight of the inner product (a common factor, it cancels in gamma)."""
+    m = len(xs) - 1
+    x, r = xs[m], rs[m]
+    new = x - beta * r
+    if m > 0:
+        for j in range(x.shape[0]):
+            dx = np.array([(xs[m - a][j] - xs[m - a - 1][j]).ravel() for a in range(m)])
+            dr = np.array([(rs[m - a][j] - rs[m - a - 1][j]).ravel() for a in range(m)])
+            gram = w * (dr.conj() @ dr.T)
+            rhs = w * (dr.conj() @ r[j].ravel())
+            gram = gram + 1e-14 * np.trace(gram).real / m * np.eye(m)
+            gamma = np.linalg.solve(gram, rhs)
+            new[j] = new[j] - ((dx - beta * dr).T @ gamma).reshape(x[j].shape)
+    return np.ascontiguousarray(new)
+
+
 def ptcn_step(model: Model, psi_n: np.ndarray, dt: float, tol: float = 1e-10, max_iter: int = 60, beta: float = 1.0,
               depth: int = 20):
     """One PT-CN step (Algorithm 1).  Returns (psi_{n+1}, info)."""
@@ -92,21 +113,11 @@ def ptcn_step(model: Model, psi_n: np.ndarray, dt: float, tol: float = 1e-10, ma
         if len(xs) > depth + 1:
             xs.pop(0)
             rs.pop(0)
-        m = len(xs) - 1
-        new = psi_f - beta * r_f                                         # line 7: Anderson mixing, per wavefunction
-        if m > 0:
-            for j in range(n_e):
-                dx = np.array([(xs[m - a][j] - xs[m - a - 1][j]).ravel() for a in range(m)])
-                dr = np.array([(rs[m - a][j] - rs[m - a - 1][j]).ravel() for a in range(m)])
-                gram = w * (dr.conj() @ dr.T)
-                rhs = w * (dr.conj() @ r_f[j].ravel())
-                gram = gram + 1e-14 * np.trace(gram).real / m * np.eye(m)
-                gamma = np.linalg.solve(gram, rhs)
-                new[j] = new[j] - ((dx - beta * dr).T @ gamma).reshape(model.n)
-        psi_f = np.ascontiguousarray(new)
+        psi_f = anderson_update(xs, rs, beta, w)                         # line 7: Anderson mixing, per wavefunction
         rho_new = oracle.density(psi_f)                                  # line 8
         change = float(np.abs(rho_new - rho).sum() * w / n_e)
         rho = rho_new
         info.update(iterations=it + 1, rho_change=change)                # line 9: the density change is reported; the
         #                                                                  residual (checked above) decides
+    info["psi_f"] = psi_f.copy()                                         # the fixed point of Eq. (5) before line 11 (for the pins)
     return oracle.orthonormalize(psi_f, w), info                         # line 11

@@ -8,7 +8,14 @@
      (no FFT), U from numpy's eigendecomposition.
   P3 the converged Psi_f satisfies Eq. (5) with the full model (exchange + density coupling), evaluated here from the
      definition; the output is orthonormal.
+     The residual of Eq. (5) is evaluated at the un-orthogonalised fixed point with H_f rebuilt from Psi_f (bar 1e-9).
   P5 kinetic operator: plane waves are eigenfunctions with eigenvalue |G|^2 / 2.
+  P6 H[Psi] Psi with exchange AND density coupling against a dense N x N matrix assembled point by point on 4^3 (explicit
+     exponentials, v(G) typed out here, no FFT): sign and weight of every term of the model Hamiltonian (Alg. 1 line 5).
+  P7 the Anderson update (Alg. 1 line 7): on linear residuals R_j(x) = A_j x - b_j of dimension d, one system
+     per wavefunction, full-depth mixing with beta = 1 reaches the exact solutions within d + 1 iterations (Krylov
+     property of Anderson's method); plain mixing does not, and neither would one least-squares problem shared by the
+     wavefunctions.
 """
 import math
 
@@ -96,19 +103,24 @@ def test_P3_fixed_point_satisfies_eq5_and_output_is_orthonormal():
     out, info = ptcn_ref.ptcn_step(model, psi0, dt=dt, tol=1e-11, max_iter=100)
     assert info["residual"] < 1e-11 and info["iterations"] < 60
     assert np.abs(oracle.overlap(out, out, model.w) - np.eye(3)).max() <= 1e-12
-    # Eq. (5) from its definition, at the un-orthogonalised fixed point: redo the iteration's last state by hand.
-    # The orthonormalised output spans the same space; Eq. (5) is covariant under unitary mixing only, so the check
-    # uses the residual the oracle reports AND an independent evaluation for a rotated copy of the fixed point.
+    # Eq. (5) from its definition (Alg. 1 lines 5-6), at the un-orthogonalised fixed point Psi_f the oracle
+    # hands out: H_f is REBUILT here from Psi_f (density and exchange operator), so an oracle that froze the Hamiltonian at
+    # Psi_n during the iteration (residual 1.8e-3 in that mutant) or dropped a term of line 6 fails the 1e-9 bar.
     def eq5_residual(pf, pn):
         def hres(p):
             hp = model.h_apply(p)
             s = model.w * np.einsum("mr,nr->mn", p.reshape(3, -1).conj(), hp.reshape(3, -1))
             return hp - np.einsum("mr,mn->nr", p.reshape(3, -1), s).reshape(p.shape)
         return pf + 0.5j * dt * hres(pf) - (pn - 0.5j * dt * hres(pn))
-    # the PT-CN solution stays orthonormal to O(dt^3) even before line 11, so `out` is within that of the fixed point
-    r = eq5_residual(out, psi0)
+    r = eq5_residual(info["psi_f"], psi0)
     nrm = math.sqrt(model.w * np.sum(np.abs(r) ** 2) / 3)
-    assert nrm < 5e-3 * dt
+    assert nrm <= 1e-9, nrm
+    # the step is not trivial: the fixed point is far (on the 1e-9 scale) from both Psi_n and the explicit half step
+    assert np.abs(info["psi_f"] - psi0).max() > 1e-3 * np.abs(psi0).max()
+    # the orthonormalised output spans the same space (line 11 only mixes the columns of Psi_f)
+    pf = info["psi_f"].reshape(3, -1)
+    proj = out.reshape(3, -1).T @ (model.w * (out.reshape(3, -1).conj() @ pf.T))       # P_out Psi_f
+    assert np.abs(proj - pf.T).max() <= 1e-11 * np.abs(pf).max()
     # and its density matrix is gauge invariant: mixing Psi_n by a unitary first gives the same P_{n+1}
     q, _ = np.linalg.qr(rng.standard_normal((3, 3)) + 1j * rng.standard_normal((3, 3)))
     out2, _ = ptcn_ref.ptcn_step(model, np.ascontiguousarray(np.einsum("mr,mn->nr", psi0.reshape(3, -1), q).reshape(psi0.shape)),
@@ -116,3 +128,62 @@ def test_P3_fixed_point_satisfies_eq5_and_output_is_orthonormal():
     p1 = out.reshape(3, -1).T @ out.reshape(3, -1).conj()
     p2 = out2.reshape(3, -1).T @ out2.reshape(3, -1).conj()
     assert np.abs(p1 - p2).max() <= 1e-8 * np.abs(p1).max()
+
+
+def test_P6_h_apply_with_exchange_and_density_coupling_matches_a_dense_matrix():
+    n, edges = (4, 4, 4), (5.0, 6.0, 7.0)
+    N = 64
+    cell = [edges[0], 0, 0, 0, edges[1], 0, 0, 0, edges[2]]
+    rng = np.random.default_rng(21)
+    v = 0.3 * rng.standard_normal(n)
+    alpha, g, omega = 0.25, 0.7, 0.106
+    psi = rng.standard_normal((3,) + n) + 1j * rng.standard_normal((3,) + n)
+    model = ptcn_ref.Model(cell, n, kernel=1, omega=omega, alpha=alpha, v_ext=v, g=g)
+    got = model.h_apply(np.ascontiguousarray(psi)).reshape(3, N)
+    # dense H[Psi] = T + diag(v + g rho) + V_X[Psi], V_X(r, r') = -alpha sum_i psi_i(r) K(r - r') conj(psi_i(r')),
+    # K(d) = (1/N) sum_G v(G) exp(i G d) (include/ptfock.h: unnormalised forward DFT, 1/N on the inverse, no volume factor)
+    P = psi.reshape(3, N)
+    rho = (np.abs(P) ** 2).sum(0)
+    H = _dense_h(edges, n, v + g * rho.reshape(n))
+    idx = np.array([(a, b, c) for a in range(4) for b in range(4) for c in range(4)])
+    K = np.zeros((N, N), dtype=complex)
+    for k0 in range(4):
+        for k1 in range(4):
+            for k2 in range(4):
+                m = [k if k < 2 else k - 4 for k in (k0, k1, k2)]
+                G2 = sum((2 * np.pi * m[d] / edges[d]) ** 2 for d in range(3))
+                vg = np.pi / omega ** 2 if G2 == 0 else 4 * np.pi / G2 * (1.0 - math.exp(-G2 / (4 * omega ** 2)))
+                ph = np.exp(2j * np.pi * (k0 * idx[:, 0] + k1 * idx[:, 1] + k2 * idx[:, 2]) / 4)
+                K += vg / N * np.outer(ph, ph.conj())
+    VX = -alpha * sum(np.outer(P[i], P[i].conj()) for i in range(3)) * K
+    ref = (H + VX) @ P.T                                               # [r, j]
+    assert np.abs(got.T - ref).max() <= 1e-12 * np.abs(ref).max()
+    # each term matters at this bar
+    assert np.abs(VX @ P.T).max() > 1e-3 * np.abs(ref).max() and np.abs(g * rho[:, None] * P.T).max() > 1e-3 * np.abs(ref).max()
+
+
+def test_P7_anderson_update_solves_linear_systems_in_d_plus_1_iterations():
+    d, n_e = 5, 3
+    rng = np.random.default_rng(33)
+    A = [np.eye(d) + 0.35 * (rng.standard_normal((d, d)) + 1j * rng.standard_normal((d, d))) / math.sqrt(d) for _ in range(n_e)]
+    b = rng.standard_normal((n_e, d)) + 1j * rng.standard_normal((n_e, d))
+    exact = np.array([np.linalg.solve(A[j], b[j]) for j in range(n_e)])
+    res = lambda x: np.array([A[j] @ x[j] - b[j] for j in range(n_e)])
+
+    def iterate(update, iters):
+        x = np.zeros((n_e, d, 1, 1), dtype=complex)                     # [n_e, grid]: the layout ptcn_step uses
+        xs, rs = [], []
+        for _ in range(iters):
+            xs.append(x.copy())
+            rs.append(res(x.reshape(n_e, d)).reshape(x.shape))
+            x = update(xs, rs)
+        return x.reshape(n_e, d)
+
+    x = iterate(lambda xs, rs: ptcn_ref.anderson_update(xs, rs, 1.0, 0.37), d + 1)
+    assert np.abs(x - exact).max() <= 1e-9 * np.abs(exact).max()
+    # plain mixing x - R(x) is nowhere near after the same number of steps: the history term does the work
+    y = iterate(lambda xs, rs: xs[-1] - rs[-1], d + 1)
+    assert np.abs(y - exact).max() > 1e-4 * np.abs(exact).max()
+    # with d iterations (history one short) the solution is not reached yet: it is the Krylov dimension that counts
+    z = iterate(lambda xs, rs: ptcn_ref.anderson_update(xs, rs, 1.0, 0.37), d - 1)
+    assert np.abs(z - exact).max() > 1e-6 * np.abs(exact).max()
