@@ -61,7 +61,8 @@ enum {
     PTFOCK_ERR_ALLOC = -5,              /* device or host allocation failed (workspace too small included) */
     PTFOCK_ERR_CUDA = -6,               /* a CUDA runtime call failed; see ptfock_last_cuda_error */
     PTFOCK_ERR_ALIAS = -7,              /* out overlaps phi or psi */
-    PTFOCK_ERR_NOT_POSITIVE = -8        /* ptfock_orthonormalize: the overlap matrix is not positive definite */
+    PTFOCK_ERR_NOT_POSITIVE = -8,       /* ptfock_orthonormalize: the overlap matrix is not positive definite */
+    PTFOCK_ERR_TOO_LARGE = -9           /* ptfock_banddot_static: n exceeds PTFOCK_STATIC_MAX_BANDS (fixed built-in scratch) */
 };
 
 typedef struct {
@@ -179,6 +180,43 @@ int ptfock_banddot(ptfock_plan *plan, const void *a, const void *b, int32_t n, d
 int ptfock_destroy(ptfock_plan *plan);
 
 /* Static string for an error code. */
+/* ---- the one entry point that allocates nothing -----------------------------------------------------------------
+ * Who needs it: a host code that cannot let this library call cudaMalloc.  Typical cases: an electronic-structure
+ * code that has handed all of HBM to its own memory pool at start-up, so that a cudaMalloc from a library simply fails;
+ * and a time-step loop whose other streams (copies, NCCL traffic) must keep running, which cudaMalloc / cudaFree
+ * would stall because both synchronise the whole device.  Such a caller cannot even build a plan (ptfock_create
+ * allocates the tables and the scratch), so this call takes NO plan.
+ *
+ * What it computes: the per-band inner products of ptfock_banddot, the entries of the per-wavefunction least-squares
+ * problems of the Anderson mixing (Sec. 3.4),
+ *     out[j] = weight * sum_{r < n_points} conj(a_j(r)) b_j(r),   j < n,
+ * by the same two kernels, summed in the same fixed order (bit-identical to ptfock_banddot on a plan with
+ * N = n_points and Omega/N = weight).  The kernels need scratch for their per-block partial sums; here it is a
+ * fixed array of PTFOCK_STATIC_MAX_BANDS * 64 complex numbers = 4 MiB built into the library image.  Every GPU
+ * that loads libptfock.so carries these 4 MiB until the process exits, whether or not this call is ever used.
+ *
+ *   device   : CUDA ordinal a, b, out live on; left as the caller's current device on return.
+ *   n_points : grid points per band (>= 1);  weight: Omega / N for the inner product of this header, or any scale.
+ *   a, b     : n bands each, [band][point] complex fp64, DEVICE, 16-byte aligned (inputs, caller-owned).
+ *   out      : n complex fp64 (re, im), DEVICE, 16-byte aligned (output, caller-owned).
+ *   n        : 1 .. PTFOCK_STATIC_MAX_BANDS; a larger n returns PTFOCK_ERR_TOO_LARGE and launches nothing (split the
+ *              bands over several calls on ONE stream instead).
+ * Asynchronous on `stream`; nothing is synchronised.  The call itself performs no cudaMalloc / cudaFree /
+ * cudaMallocHost and calls no library routine that allocates.
+ *
+ * First call on each device: the library looks up the device address of its built-in array (one
+ * cudaGetSymbolAddress with that device current; this may also make the CUDA runtime load the library's kernels onto
+ * the device) and remembers it.  Make that first call during start-up, before any stream capture begins; later calls
+ * only launch the two kernels.
+ *
+ * Sharing: all calls on a device, from every thread and stream, use the SAME array, and it keeps whatever the last
+ * call left in it.  Nothing in it has to start at zero: each call overwrites every partial sum before it reads it.
+ * Two calls that can overlap on the GPU (different streams without an event between them) race on the array and give
+ * wrong results; calls on one stream, or ordered by events, are safe. */
+#define PTFOCK_STATIC_MAX_BANDS 4096
+int ptfock_banddot_static(int32_t device, int64_t n_points, double weight, const void *a, const void *b, int32_t n,
+                          void *out, void *stream);
+
 const char *ptfock_strerror(int code);
 
 /* The cudaError_t of the most recent PTFOCK_ERR_CUDA on this thread (0 if none). */

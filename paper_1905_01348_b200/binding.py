@@ -25,7 +25,8 @@ EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_ap
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
            "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_dmma_peak", "ptfock_measure_copy_bandwidth",
            "ptfock_overlap", "ptfock_rotate", "ptfock_residual", "ptfock_density", "ptfock_orthonormalize",
-           "ptfock_hloc_apply", "ptfock_axpby", "ptfock_banddot"]
+           "ptfock_hloc_apply", "ptfock_axpby", "ptfock_banddot", "ptfock_banddot_static"]
+STATIC_MAX_BANDS = 4096
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "1886"]
@@ -92,6 +93,7 @@ def lib() -> ctypes.CDLL:
         L.ptfock_hloc_apply.argtypes = [vp, vp, vp, i32, vp, vp]
         L.ptfock_axpby.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
         L.ptfock_banddot.argtypes = [vp, vp, vp, i32, vp, vp]
+        L.ptfock_banddot_static.argtypes = [i32, ctypes.c_int64, ctypes.c_double, vp, vp, i32, vp, vp]
         for name in EXPORTS:
             if name != "ptfock_strerror":
                 getattr(L, name).restype = ctypes.c_int
@@ -343,6 +345,26 @@ class Plan:
 
     def __exit__(self, *a):
         self.destroy()
+
+
+def banddot_static(a, b, weight: float, out=None):
+    """out[j] = weight * sum_r conj(a_j(r)) b_j(r) through ptfock_banddot_static: no plan, and no allocation inside the
+    library (its partial sums live in a fixed 4 MiB array built into libptfock.so), for host codes that own all device
+    memory themselves or cannot afford cudaMalloc's device-wide stall.  ``a``, ``b``: [n, ...] complex128 CUDA tensors,
+    n <= STATIC_MAX_BANDS; ``out``: optional complex128 CUDA tensor of n numbers (pass it to keep torch from allocating
+    too).  Asynchronous on torch's current stream; calls that may overlap on the GPU race on the shared array."""
+    import torch
+    if not (isinstance(a, torch.Tensor) and isinstance(b, torch.Tensor) and a.is_cuda and a.dim() >= 2 and a.shape == b.shape):
+        raise TypeError("a and b must be CUDA tensors of the same shape [n, ...]")
+    dev = a.device.index
+    n = a.shape[0]
+    if out is None:
+        out = torch.empty(n, dtype=torch.complex128, device=a.device)
+    elif out.numel() != n:
+        raise ValueError("out must hold n complex numbers")
+    _check(lib().ptfock_banddot_static(dev, a[0].numel(), float(weight), _dev_ptr(a, "a", dev), _dev_ptr(b, "b", dev), n,
+                                       _dev_ptr(out, "out", dev), _stream(dev)), "ptfock_banddot_static")
+    return out
 
 
 def measure_fp64_peak(device: int = 0) -> float:

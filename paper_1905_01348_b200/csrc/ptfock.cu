@@ -16,6 +16,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <initializer_list>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -599,6 +600,7 @@ extern "C" const char *ptfock_strerror(int code) {
         default: return "unknown error";
     }
 }
+        case PTFOCK_ERR_TOO_LARGE: return "too many bands for the built-in scratch (ptfock_banddot_static: n <= PTFOCK_STATIC_MAX_BANDS = 4096; split the call)";
 
 extern "C" int ptfock_last_cuda_error(void) { return g_last_cuda; }
 
@@ -1412,6 +1414,60 @@ int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host) {
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(sink);
+// ---- ptfock_banddot_static: the same two kernels with their partial sums in a built-in array (no allocation) ----------
+// For callers that must not trigger a cudaMalloc (all HBM owned by their own pool, or a loop whose other streams a
+// device-wide synchronising allocation would stall); see include/ptfock.h.
+namespace {
+constexpr int kStaticBlocksPer = 64;                                    // the most blocks per band banddot_partial is launched with
+constexpr int kStaticMaxDevices = 64;
+// Per-block partial sums of one call: [band][block].  One copy per GPU that loads the library (4 MiB), alive until exit.
+// Host code must NOT hand this name to a kernel: on the host it is only a handle for cudaGetSymbolAddress.
+static __device__ __align__(256) double2 g_banddot_static_part[(size_t)PTFOCK_STATIC_MAX_BANDS * kStaticBlocksPer];
+double2 *g_static_part_addr[kStaticMaxDevices] = {};                    // device address of the array, per ordinal (0 = not looked up yet)
+std::mutex g_static_mu;
+
+// `device` is current.  Looks the array's device address up once per device; no allocation.
+int static_part_address(int device, double2 **out) {
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_part_addr[device]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_banddot_static_part));
+        if (!p) return PTFOCK_ERR_CUDA;
+        g_static_part_addr[device] = static_cast<double2 *>(p);
+    }
+    *out = g_static_part_addr[device];
+    return PTFOCK_OK;
+}
+}  // namespace
+
+extern "C" int ptfock_banddot_static(int32_t device, int64_t n_points, double weight, const void *a, const void *b, int32_t n,
+                                     void *out, void *stream) {
+    if (!a || !b || !out || n < 1 || n_points < 1 || device < 0 || device >= kStaticMaxDevices) return PTFOCK_ERR_INVALID_ARG;
+    if (n > PTFOCK_STATIC_MAX_BANDS) return PTFOCK_ERR_TOO_LARGE;
+    int count = 0;
+    CU(cudaGetDeviceCount(&count));
+    if (device >= count) return PTFOCK_ERR_INVALID_ARG;
+    for (const void *q : { a, b, (const void *)out }) {
+        if ((uintptr_t)q & 15) return PTFOCK_ERR_ALIGNMENT;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, q) != cudaSuccess) { cudaGetLastError(); return PTFOCK_ERR_INVALID_ARG; }
+        if (at.type == cudaMemoryTypeManaged) continue;
+        if (at.type != cudaMemoryTypeDevice || at.device != device) return PTFOCK_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(device);
+    double2 *part = nullptr;
+    int rc = static_part_address(device, &part);                        // first call on this device: cudaGetSymbolAddress
+    if (rc != PTFOCK_OK) return rc;
+    // same launch shape as ptfock_banddot, so the sums are taken in the same order; every part[j][0 .. blocks_per) that
+    // banddot_final reads is written by banddot_partial first, so what an earlier call left in the array does not matter
+    const int blocks_per = (int)std::max<long long>(1, std::min<long long>(kStaticBlocksPer, n_points / 2048));
+    banddot_partial<<<dim3(blocks_per, n), 256, 0, st>>>((const cd *)a, (const cd *)b, n_points, blocks_per, part);
+    banddot_final<<<(n + 63) / 64, 64, 0, st>>>(part, blocks_per, n, weight, (double2 *)out);
+    CU(cudaGetLastError());
+    return PTFOCK_OK;
+}
+
     *tflops_host = best;
     return PTFOCK_OK;
 }
