@@ -1,8 +1,8 @@
 // slabx.cuh -- TMA-fed, in-place slab passes (pass A and pass C of the BASELINE shapes 64x64 and 128x48).
 //
-// Same three butterfly stages per (x1, x2) slab as slab2.cuh, re-ordered so that every byte that crosses
-// the L1/shared-memory pipe is useful (ncu on the slab2 kernels: the LSU data pipe is the busiest unit,
-// and its orbital loads touched only half of every 128-byte line):
+// Same three butterfly stages per (x1, x2) slab as the generic slab passes of kernels.cuh, ordered so that every byte
+// that crosses the L1/shared-memory pipe is useful (ncu on a round-1 predecessor of these kernels: the LSU data pipe
+// was the busiest unit, and its orbital loads touched only half of every 128-byte line):
 //
 //   * x1 is transformed FIRST and x2 LAST.  Stage 1 threads own points that are consecutive in x2, so the
 //     psi_j / phi_i / out accesses of Eq. (3)'s products (Alg. 2 lines 7-9,
