@@ -78,7 +78,10 @@ typedef struct {
     int32_t device;           /* CUDA ordinal                                                               */
     int32_t block_i;          /* pair-scheduler tile: orbitals i per wave (0 = library chooses)            */
     int32_t block_j;          /* pair-scheduler tile: targets j per wave  (0 = library chooses)            */
-    uint64_t workspace_bytes; /* upper bound for the pair-density scratch (0 = library chooses)            */
+    uint64_t workspace_bytes; /* upper bound for the scratch (0 = library chooses, and never below what the
+                                 dense-algebra calls need for max(n_occ, max_targets) orbitals); with a bound
+                                 the scratch never exceeds it and a dense-algebra call that needs more returns
+                                 PTFOCK_ERR_ALLOC                                                            */
     uint32_t flags;           /* PTFOCK_FLAG_* (0 = library chooses the kernels)                            */
 } ptfock_desc;
 
@@ -167,8 +170,9 @@ int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, void *stream)
 int ptfock_hloc_apply(ptfock_plan *plan, const double *vloc, const void *psi, int32_t n, void *out, void *stream);
 
 /* out_j = a_j x_j + b_j y_j, j < n, with per-orbital complex coefficients from HOST arrays of n (re, im) pairs (the mixing
- * coefficients of PAPER.md:194 are per wavefunction); y and b_host may be NULL.  out may be x or y.  Asynchronous; the
- * host arrays may be reused when the call returns. */
+ * coefficients of PAPER.md:194 are per wavefunction); y and b_host may be NULL.  out may be x or y.  Asynchronous, with
+ * no copy and no synchronisation: the coefficients are passed to the kernels by value (64 orbitals per launch), so the
+ * host arrays, pinned or pageable, may be reused when the call returns. */
 int ptfock_axpby(ptfock_plan *plan, int32_t n, const double *a_host, const void *x, const double *b_host, const void *y,
                  void *out, void *stream);
 
@@ -176,10 +180,23 @@ int ptfock_axpby(ptfock_plan *plan, int32_t n, const double *a_host, const void 
  * per-wavefunction least-squares problems of the Anderson mixing.  Synchronises `stream`. */
 int ptfock_banddot(ptfock_plan *plan, const void *a, const void *b, int32_t n, double *out_host, void *stream);
 
-/* Frees everything the plan owns.  NULL is allowed. */
-int ptfock_destroy(ptfock_plan *plan);
+/* out_host[k * n + j] = (a_j, b^k_j), k < n_sets, j < n: ptfock_banddot of one orbital set `a` against n_sets others in one
+ * call with one synchronisation -- a new row of the per-wavefunction Gram matrices of the Anderson mixing, or their
+ * right-hand sides ("evaluation of overlap matrices").  b_sets_host: HOST array of n_sets DEVICE
+ * pointers (n orbitals each); out_host: n_sets * n (re, im) pairs, HOST.  Same kernels and summation order as
+ * ptfock_banddot (bit-identical per set).  Synchronises `stream`. */
+int ptfock_banddot_many(ptfock_plan *plan, const void *a, const void *const *b_sets_host, int32_t n_sets, int32_t n,
+                        double *out_host, void *stream);
 
-/* Static string for an error code. */
+/* v_out(r) = v_ext(r) + g rho(r): the local potential of the model Hamiltonian following the density (Alg. 1 line 5,
+ * PAPER.md:84 "Update the potential").  v_ext (NULL = 0), rho, v_out: N doubles, DEVICE; v_out may be v_ext or rho.
+ * Asynchronous. */
+int ptfock_vloc_update(ptfock_plan *plan, const double *v_ext, double g, const double *rho, double *v_out, void *stream);
+
+/* *change_host = (Omega/N) sum_r |rho_a(r) - rho_b(r)|: the density change between two SCF iterations that Alg. 1 line 9
+ * monitors.  rho_a, rho_b: N doubles, DEVICE; change_host: HOST.  Deterministic; synchronises `stream`. */
+int ptfock_density_change(ptfock_plan *plan, const double *rho_a, const double *rho_b, double *change_host, void *stream);
+
 /* ---- the one entry point that allocates nothing -----------------------------------------------------------------
  * Who needs it: a host code that cannot let this library call cudaMalloc.  Typical cases: an electronic-structure
  * code that has handed all of HBM to its own memory pool at start-up, so that a cudaMalloc from a library simply fails;
@@ -220,6 +237,10 @@ int ptfock_banddot_static(int32_t device, int64_t n_points, double weight, const
 const char *ptfock_strerror(int code);
 
 /* The cudaError_t of the most recent PTFOCK_ERR_CUDA on this thread (0 if none). */
+/* Frees everything the plan owns.  NULL is allowed. */
+int ptfock_destroy(ptfock_plan *plan);
+
+/* Static string for an error code. */
 int ptfock_last_cuda_error(void);
 
 /* Introspection for the harness (host memory, no device work):
@@ -227,7 +248,7 @@ int ptfock_last_cuda_error(void);
  *   issued by the most recent apply, info[4] = pair-solves executed by the most recent apply,
  *   info[5] = 1 if the most recent apply used the symmetric schedule, info[6] = total launches since create,
  *   info[7] = kernel family in the low 4 bits: 0 three-stage slab passes + pencil pass, 1 two-stage slab passes +
- *             32 x 32 pencil pass (64^3), 2 single-pass on-chip kernel (16^3); bit 4 (value 16) set if the scratch
+ *             two-stage pencil pass (64^3, 48^3, 32^3), 2 single-pass on-chip kernel (16^3); bit 4 (value 16) set if the scratch
  *             holds two waves (two waves in flight on the general schedule). */
 int ptfock_plan_info(const ptfock_plan *plan, int64_t info[8]);
 

@@ -25,7 +25,8 @@ EXPORTS = ["ptfock_create", "ptfock_apply", "ptfock_exchange_energy", "ptfock_ap
            "ptfock_strerror", "ptfock_last_cuda_error", "ptfock_plan_info", "ptfock_debug_pair",
            "ptfock_set_profiling", "ptfock_get_profile", "ptfock_measure_dfma_peak", "ptfock_measure_dmma_peak", "ptfock_measure_copy_bandwidth",
            "ptfock_overlap", "ptfock_rotate", "ptfock_residual", "ptfock_density", "ptfock_orthonormalize",
-           "ptfock_hloc_apply", "ptfock_axpby", "ptfock_banddot", "ptfock_banddot_static"]
+           "ptfock_hloc_apply", "ptfock_axpby", "ptfock_banddot", "ptfock_banddot_static",
+           "ptfock_banddot_many", "ptfock_vloc_update", "ptfock_density_change"]
 STATIC_MAX_BANDS = 4096
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -93,6 +94,9 @@ def lib() -> ctypes.CDLL:
         L.ptfock_hloc_apply.argtypes = [vp, vp, vp, i32, vp, vp]
         L.ptfock_axpby.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
         L.ptfock_banddot.argtypes = [vp, vp, vp, i32, vp, vp]
+        L.ptfock_banddot_many.argtypes = [vp, vp, ctypes.POINTER(vp), i32, i32, vp, vp]
+        L.ptfock_vloc_update.argtypes = [vp, vp, ctypes.c_double, vp, vp, vp]
+        L.ptfock_density_change.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
         L.ptfock_banddot_static.argtypes = [i32, ctypes.c_int64, ctypes.c_double, vp, vp, i32, vp, vp]
         for name in EXPORTS:
             if name != "ptfock_strerror":
@@ -313,6 +317,44 @@ class Plan:
         _check(lib().ptfock_banddot(self._h, _dev_ptr(a, "a", self.device), _dev_ptr(b, "b", self.device), n,
                                     ctypes.c_void_p(res.ctypes.data), _stream(self.device)), "ptfock_banddot")
         return res
+
+    def banddot_many(self, a, b_sets):
+        """numpy array [len(b_sets), n] of (a_j, b^k_j) in one call (one synchronisation)."""
+        import numpy as np
+        n = self._grids(a, "a")
+        ptrs = (ctypes.c_void_p * len(b_sets))(*[_dev_ptr(b, "b_sets[k]", self.device).value for b in b_sets])
+        for b in b_sets:
+            if self._grids(b, "b_sets[k]") != n:
+                raise ValueError("every set must hold as many orbitals as a")
+        res = np.empty((len(b_sets), n), dtype=np.complex128)
+        _check(lib().ptfock_banddot_many(self._h, _dev_ptr(a, "a", self.device), ptrs, len(b_sets), n,
+                                         ctypes.c_void_p(res.ctypes.data), _stream(self.device)), "ptfock_banddot_many")
+        return res
+
+    def _real_grid(self, t, what):
+        import torch
+        if t is None:
+            return ctypes.c_void_p(0)
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and t.numel() == self.N and t.device.index == self.device):
+            raise TypeError(f"{what} must be a contiguous float64 CUDA tensor of one grid on cuda:{self.device}")
+        return ctypes.c_void_p(t.data_ptr())
+
+    def vloc_update(self, v_ext, g: float, rho, out=None):
+        """v_ext + g rho on the device (Alg. 1 line 5)."""
+        import torch
+        if out is None:
+            out = torch.empty_like(rho)
+        _check(lib().ptfock_vloc_update(self._h, self._real_grid(v_ext, "v_ext"), float(g), self._real_grid(rho, "rho"),
+                                        self._real_grid(out, "out"), _stream(self.device)), "ptfock_vloc_update")
+        return out
+
+    def density_change(self, rho_a, rho_b) -> float:
+        """(Omega/N) sum_r |rho_a - rho_b| (Alg. 1 line 9)."""
+        v = ctypes.c_double(0.0)
+        _check(lib().ptfock_density_change(self._h, self._real_grid(rho_a, "rho_a"), self._real_grid(rho_b, "rho_b"),
+                                           ctypes.byref(v), _stream(self.device)), "ptfock_density_change")
+        return v.value
 
     def info(self) -> dict:
         a = (ctypes.c_int64 * 8)()

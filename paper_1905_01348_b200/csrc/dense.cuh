@@ -21,20 +21,25 @@ struct OverlapArgs {
     cd *part;               // [k_splits][n_a][ld]
     long long n_pts, pts_per_split;
     int n_a, n_b, ld;       // ld = row pitch of part / S (>= n_b)
+    int lower;              // 1: a == b (Hermitian product): gridDim.x counts the 64 x 64 tiles tm >= tn only, the tiles above
+                            //    the diagonal are never computed (overlap_reduce mirrors them)
 };
 
-// s[m][n] = w * sum_ks part[ks][m][n] (fixed order)
+// s[m][n] = w * sum_ks part[ks][m][n] (fixed order); herm: entries of the tiles above the diagonal are the conjugates of
+// their mirror images (those tiles hold no partial sums)
 __global__ void __launch_bounds__(256) overlap_reduce(const cd *part, int k_splits, int n_a, int n_b, int ld_part, double w,
-                                                      cd *s, int ld_s) {
+                                                      cd *s, int ld_s, int herm) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= (long long)n_a * n_b) return;
     const int m = (int)(k / n_b), n = (int)(k % n_b);
-    cd t = part[(long long)m * ld_part + n];
+    const bool mirror = herm && (m >> 6) < (n >> 6);
+    const int row = mirror ? n : m, col = mirror ? m : n;
+    cd t = part[(long long)row * ld_part + col];
     for (int q = 1; q < k_splits; ++q) {
-        const cd u = part[((long long)q * n_a + m) * ld_part + n];
+        const cd u = part[((long long)q * n_a + row) * ld_part + col];
         t.x += u.x; t.y += u.y;
     }
-    s[(long long)m * ld_s + n] = make_double2(t.x * w, t.y * w);
+    s[(long long)m * ld_s + n] = make_double2(t.x * w, mirror ? -t.y * w : t.y * w);
 }
 
 // ---- rotation with fused epilogues: acc_n(r) = sum_m a_m(r) c(m, n) ---------------------------------------------------

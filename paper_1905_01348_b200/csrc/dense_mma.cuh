@@ -42,7 +42,8 @@ __global__ void __launch_bounds__(256) dmma_peak_kernel(double *sink, int iters,
 }
 
 // ---- overlap: part[ks][m][n] = sum over this split's points of conj(a[m][r]) b[n][r] ------------------------------------
-// grid = (ceil(n_a / 64), ceil(n_b / 64), k_splits); 128 threads = 2 x 2 warps, warp tile 32 x 32 = 4 x 4 DMMA tiles for
+// grid = (ceil(n_a / 64), ceil(n_b / 64), k_splits), or (T (T + 1) / 2, 1, k_splits) lower-triangle tiles for a Hermitian
+// product (OverlapArgs::lower); 128 threads = 2 x 2 warps, warp tile 32 x 32 = 4 x 4 DMMA tiles for
 // the real and 4 x 4 for the imaginary part (128 accumulator registers).  K advances 16 points per stage through a
 // 3-stage cp.async ring; a tile row is 16 points = 256 bytes + 32 bytes of padding: the fragment reads (8 rows x 32
 // bytes for A, 8 rows x 2 complex elements for B) then touch every bank exactly once per 128-byte wavefront.
@@ -57,7 +58,14 @@ __global__ void __launch_bounds__(128, 2) overlap_mma(const OverlapArgs g) {
     cd *ring = reinterpret_cast<cd *>(dense_smem);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
-    const int m0 = blockIdx.x * 64, n0 = blockIdx.y * 64;
+    int tm = blockIdx.x, tn = blockIdx.y;
+    if (g.lower) {                                         // blockIdx.x = tm (tm + 1) / 2 + tn with tn <= tm
+        tm = (int)((sqrt(8.0 * (double)blockIdx.x + 1.0) - 1.0) * 0.5);
+        while ((tm + 1) * (tm + 2) / 2 <= (int)blockIdx.x) ++tm;
+        while (tm * (tm + 1) / 2 > (int)blockIdx.x) --tm;
+        tn = (int)blockIdx.x - tm * (tm + 1) / 2;
+    }
+    const int m0 = tm * 64, n0 = tn * 64;
     const long long r_beg = (long long)blockIdx.z * g.pts_per_split;
     const long long r_end = min(g.n_pts, r_beg + g.pts_per_split);
     const int n_steps = (int)((r_end - r_beg + kMK - 1) / kMK);

@@ -429,17 +429,26 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
     const int gi = threadIdx.x / S::NTB, tid = threadIdx.x % S::NTB;       // group, thread in group
     const int pair = blockIdx.y * GB + gi;
     cd *s = reinterpret_cast<cd *>(smem_b + gi * S::TILE_B);
+    // pair pr of the wave is solved unless it lies past the wave's end or above the diagonal of a triangular block
+    auto live = [&](int pr) { return pr < g.n_pairs && !(g.tri_nj > 0 && pr / g.tri_nj > pr % g.tri_nj); };
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int k = 0; k <= GB; ++k) mbar_init(&bars[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
-        mbar_expect_tx(&bars[GB], S::V_BYTES);
-        bulk_g2s(smem_b + GB * S::TILE_B, g.v + (long long)grp_pos * (S::V_BYTES / 16), S::V_BYTES, &bars[GB]);
+        bool any = false;
+#pragma unroll
+        for (int k = 0; k < GB; ++k) any |= live(blockIdx.y * GB + k);
+        // a CTA whose GB pairs are all skipped (e.g. pairs (3,0) (3,1) (3,2) of a triangular block) returns below without
+        // waiting on anything: it must not leave a bulk copy and its complete_tx in flight into shared memory that the
+        // SM's next CTA may already own.  With one live group, that group waits for v' before the CTA can exit.
+        if (any) {
+            mbar_expect_tx(&bars[GB], S::V_BYTES);
+            bulk_g2s(smem_b + GB * S::TILE_B, g.v + (long long)grp_pos * (S::V_BYTES / 16), S::V_BYTES, &bars[GB]);
+        }
 #pragma unroll
         for (int k = 0; k < GB; ++k)
-            if (blockIdx.y * GB + k < g.n_pairs &&
-                !(g.tri_nj > 0 && (int)(blockIdx.y * GB + k) / g.tri_nj > (int)(blockIdx.y * GB + k) % g.tri_nj)) {
+            if (live(blockIdx.y * GB + k)) {
                 mbar_expect_tx(&bars[k], S::TILE_B);
                 tensor_g2s_2d_sw(smem_b + k * S::TILE_B, &map, grp_pos * (P * RQ * 2), (g.pair0 + blockIdx.y * GB + k) * S::ROWS, &bars[k]);
             }
@@ -455,7 +464,7 @@ __global__ void __maxnreg__(S::MAXREG_B) p8_mid(const __grid_constant__ CUtensor
     const int mr = t2 % RQ, mp = (t2 / RQ) % P, mq = (t2 / (RQ * P)) % NQ, mk = t2 / (RQ * P * NQ);
     const int rb = (mq * N0 + mk * B0) * 8, mc = mp * RQ + mr;
     __syncthreads();                                    // mbarrier inits visible; from here on the groups are independent
-    if (pair >= g.n_pairs || (g.tri_nj > 0 && pair / g.tri_nj > pair % g.tri_nj)) return;
+    if (!live(pair)) return;
     auto group_sync = [&]() {                           // named barrier 1 + gi over the group's threads
         if (gi == 0) asm volatile("bar.sync 1, %0;" ::"n"(S::NTB) : "memory");
         else if (gi == 1) asm volatile("bar.sync 2, %0;" ::"n"(S::NTB) : "memory");

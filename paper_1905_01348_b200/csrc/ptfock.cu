@@ -514,7 +514,10 @@ extern "C" int ptfock_create(const ptfock_desc *desc, ptfock_plan **out) {
     int slots = (!(d.flags & PTFOCK_FLAG_SINGLE_STREAM) && !p->onchip && 2 * (size_t)Ib * Jb * pair_bytes <= limit &&
                  2LL * Ib * Jb <= 65535) ? 2 : 1;
     for (;;) {
-        p->scratch_bytes = std::max((size_t)slots * Ib * Jb * pair_bytes, dense_min);
+        // with a caller's bound the dense-algebra minimum is clipped to it (those calls return PTFOCK_ERR_ALLOC when the
+        // scratch is too small for them); without one the scratch is never sized below it
+        p->scratch_bytes = std::max((size_t)slots * Ib * Jb * pair_bytes,
+                                    d.workspace_bytes ? std::min(dense_min, (size_t)d.workspace_bytes) : dense_min);
         cudaError_t e = cudaMalloc(&p->scratch, p->scratch_bytes);
         if (e == cudaSuccess) break;
         cudaGetLastError();
@@ -651,6 +654,17 @@ cudaError_t end_call(ptfock_plan *p, cudaStream_t st) {
 // profiling: record an event that closes an interval of kind `tag` (-1: opens a new run of intervals)
 void mark(Wave &w, int tag) {
     ptfock_plan *p = w.p;
+// an error return after begin_call may already have queued work on `st` (a first-use fill, part of a wave): the busy
+// event is recorded on EVERY way out, so that the next call on another stream is still ordered behind it
+struct CallScope {
+    ptfock_plan *p;
+    cudaStream_t st;
+    bool closed;
+    cudaError_t close() { closed = true; return end_call(p, st); }
+    ~CallScope() { if (!closed) end_call(p, st); }
+};
+#define BEGIN_CALL(plan_, st_) CU(begin_call(plan_, st_)); CallScope call_scope__{ plan_, st_, false }
+#define END_CALL() CU(call_scope__.close())
     if (!p->profiling) return;
     if (!p->ev_pool) { p->ev_pool = new std::vector<cudaEvent_t>(); p->ev_tags = new std::vector<int>(); }
     if (p->ev_used == p->ev_pool->size()) {
@@ -924,9 +938,9 @@ extern "C" int ptfock_apply(ptfock_plan *plan, const void *phi, const void *psi,
     if (rc != PTFOCK_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     rc = apply_device(plan, (const cd *)phi, (const cd *)psi, self_offset, n_targets, (cd *)out, st);
-    CU(end_call(plan, st));
+    END_CALL();
     return rc;
 }
 
@@ -938,7 +952,7 @@ extern "C" int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const 
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
     if (n_targets == 0) { *e_host = 0.0; return PTFOCK_OK; }
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     const cd *vx = (const cd *)vx_psi;
     if (!vx) {
         if (n_targets > plan->d.max_targets) return PTFOCK_ERR_INVALID_ARG;
@@ -959,7 +973,7 @@ extern "C" int ptfock_exchange_energy(ptfock_plan *plan, const void *phi, const 
     plan->total_launches += 2;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(plan->result_host, plan->result_dev, sizeof(double2), cudaMemcpyDeviceToHost, st));
-    CU(end_call(plan, st));
+    END_CALL();
     CU(cudaStreamSynchronize(st));
     *e_host = plan->result_host->x;
     return PTFOCK_OK;
@@ -1003,7 +1017,7 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     }
     hp.ev = plan->copy_ev;
     for (int k = 0; k < 2; ++k) { hp.waited[k].assign(hp.n_chunks, 0); hp.waited_psi[k].assign(hp.n_jchunks, 0); }
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     // the copy stream starts after whatever the caller queued on `stream`
     CU(cudaEventRecord((*hp.ev)[hp.n_chunks], st));
     CU(cudaStreamWaitEvent(hp.cs, (*hp.ev)[hp.n_chunks], 0));
@@ -1037,7 +1051,7 @@ extern "C" int ptfock_apply_host(ptfock_plan *plan, const void *phi_host, const 
     rc = apply_device(plan, plan->st_phi, psi_host ? plan->st_psi : nullptr, self_offset, n_targets, plan->st_out, st, &hp);
     if (rc != PTFOCK_OK) { cudaStreamSynchronize(hp.cs); cudaStreamSynchronize(st); return rc; }
     if (!hp.out_streamed) CUH(cudaMemcpyAsync(out_host, plan->st_out, gbytes * n_targets, cudaMemcpyDeviceToHost, st));
-    CUH(end_call(plan, st));
+    CUH(call_scope__.close());
     CUH(cudaStreamSynchronize(st));
     CUH(cudaStreamSynchronize(hp.cs));
     return PTFOCK_OK;
@@ -1050,7 +1064,7 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
     const size_t gbytes = sizeof(cd) * (size_t)plan->N;
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     if (!plan->ones) {
         cudaError_t e = cudaMalloc(&plan->ones, gbytes);
         if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
@@ -1068,7 +1082,7 @@ extern "C" int ptfock_debug_pair(ptfock_plan *plan, const void *phi_i, const voi
     plan->total_launches += w.launches + 1;
     w.note(cudaGetLastError());
     if (w.err != cudaSuccess) { g_last_cuda = (int)w.err; return PTFOCK_ERR_CUDA; }
-    CU(end_call(plan, st));
+    END_CALL();
     return PTFOCK_OK;
 }
 
@@ -1089,10 +1103,24 @@ int check_dev_ptrs(const ptfock_plan *p, std::initializer_list<const void *> ptr
     return PTFOCK_OK;
 }
 
-// S (n_a x n_b, row pitch ld_s) = w * A^H B; split-K partial sums go to `work` (bytes available: work_bytes)
+// the same for an array of doubles (rho, vloc): 8-byte alignment
+int check_dev_doubles(const ptfock_plan *p, const double *q) {
+    if (!q) return PTFOCK_OK;
+    if ((uintptr_t)q & 7) return PTFOCK_ERR_ALIGNMENT;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, q) != cudaSuccess) { cudaGetLastError(); return PTFOCK_ERR_INVALID_ARG; }
+    if (at.type == cudaMemoryTypeManaged) return PTFOCK_OK;
+    return (at.type == cudaMemoryTypeDevice && at.device == p->d.device) ? PTFOCK_OK : PTFOCK_ERR_INVALID_ARG;
+}
+
+// S (n_a x n_b, row pitch ld_s) = w * A^H B; split-K partial sums go to `work` (bytes available: work_bytes).
+// A Hermitian product (same orbitals on both sides, "Psi^* Psi") computes the 64 x 64 tiles on and below the
+// diagonal only -- half of the 8 N n^2 flops -- and mirrors the rest.
 int overlap_into(ptfock_plan *p, const cd *a, int n_a, const cd *b, int n_b, cd *s, int ld_s, cd *work, size_t work_bytes,
                  cudaStream_t st) {
-    const int tiles = ((n_a + kDT - 1) / kDT) * ((n_b + kDT - 1) / kDT);
+    const bool herm = a == b && n_a == n_b;
+    const int ta = (n_a + kDT - 1) / kDT, tb = (n_b + kDT - 1) / kDT;
+    const int tiles = herm ? ta * (ta + 1) / 2 : ta * tb;
     // split K so that the CTAs fill whole rounds of the 2 x sm_count resident CTAs: the split with the least
     // (rounds / splits) wins, the smaller one on a tie (1024 orbitals: 256 tiles x 8 splits = 6.9 rounds)
     const size_t per = sizeof(cd) * (size_t)n_a * n_b;
@@ -1112,10 +1140,10 @@ int overlap_into(ptfock_plan *p, const cd *a, int n_a, const cd *b, int n_b, cd 
     pps = (pps + kDK - 1) / kDK * kDK;
     ks = (p->N + pps - 1) / pps;
     OverlapArgs g;
-    g.a = a; g.b = b; g.part = work; g.n_pts = p->N; g.pts_per_split = pps; g.n_a = n_a; g.n_b = n_b; g.ld = n_b;
-    overlap_mma<<<dim3((n_a + kDT - 1) / kDT, (n_b + kDT - 1) / kDT, (unsigned)ks), 128, kOverlapMmaSmem, st>>>(g);
+    g.a = a; g.b = b; g.part = work; g.n_pts = p->N; g.pts_per_split = pps; g.n_a = n_a; g.n_b = n_b; g.ld = n_b; g.lower = herm ? 1 : 0;
+    overlap_mma<<<herm ? dim3(tiles, 1, (unsigned)ks) : dim3(ta, tb, (unsigned)ks), 128, kOverlapMmaSmem, st>>>(g);
     const long long cnt = (long long)n_a * n_b;
-    overlap_reduce<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(work, (int)ks, n_a, n_b, n_b, p->volume / (double)p->N, s, ld_s);
+    overlap_reduce<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(work, (int)ks, n_a, n_b, n_b, p->volume / (double)p->N, s, ld_s, herm ? 1 : 0);
     p->total_launches += 2;
     return PTFOCK_OK;
 }
@@ -1133,11 +1161,11 @@ extern "C" int ptfock_overlap(ptfock_plan *plan, const void *a, int32_t n_a, con
     if (rc != PTFOCK_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     rc = overlap_into(plan, (const cd *)a, n_a, (const cd *)b, n_b, (cd *)s, n_b, plan->scratch, plan->scratch_bytes, st);
     if (rc != PTFOCK_OK) return rc;
     CU(cudaGetLastError());
-    CU(end_call(plan, st));
+    END_CALL();
     return PTFOCK_OK;
 }
 
@@ -1167,7 +1195,7 @@ extern "C" int ptfock_residual(ptfock_plan *plan, const void *psi, const void *h
     if (s_bytes * 2 > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     cd *S = plan->scratch;
     rc = overlap_into(plan, (const cd *)psi, n, (const cd *)hpsi, n, S, n, plan->scratch + (size_t)n * n,
                       plan->scratch_bytes - s_bytes, st);                          // Alg. 3 lines 2-3
@@ -1179,7 +1207,7 @@ extern "C" int ptfock_residual(ptfock_plan *plan, const void *psi, const void *h
     g.fx = 0.0; g.fy = 0.5 * dt;                                                   // f = i dt / 2
     rotate_launch(plan, g, st);                                                    // Alg. 3 lines 4-5 fused
     CU(cudaGetLastError());
-    CU(end_call(plan, st));
+    END_CALL();
     return PTFOCK_OK;
 }
 
@@ -1187,10 +1215,11 @@ extern "C" int ptfock_density(ptfock_plan *plan, const void *psi, int32_t n, dou
     if (!plan || !psi || !rho || n < 1) return PTFOCK_ERR_INVALID_ARG;
     int rc = check_dev_ptrs(plan, { psi });
     if (rc != PTFOCK_OK) return rc;
-    if ((uintptr_t)rho & 7) return PTFOCK_ERR_ALIGNMENT;
+    rc = check_dev_doubles(plan, rho);
+    if (rc != PTFOCK_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     const long long blocks = (plan->N + 255) / 256;
     int splits = (int)std::max<long long>(1, std::min<long long>(n, (8LL * plan->sm_count + blocks - 1) / blocks));
     splits = (int)std::min<size_t>((size_t)splits, plan->scratch_bytes / (sizeof(double) * (size_t)plan->N));
@@ -1202,7 +1231,7 @@ extern "C" int ptfock_density(ptfock_plan *plan, const void *psi, int32_t n, dou
     density_reduce<<<(unsigned)blocks, 256, 0, st>>>(part, plan->N, splits, rho);
     plan->total_launches += 2;
     CU(cudaGetLastError());
-    CU(end_call(plan, st));
+    END_CALL();
     return PTFOCK_OK;
 }
 
@@ -1215,13 +1244,17 @@ extern "C" int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, vo
     if (s_bytes + sizeof(cd) * (size_t)n * n > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    if (!plan->chol_info) {
+    if (!plan->chol_info || !plan->chol_info_host) {                    // either allocation may have failed in an earlier call
         CU(cudaFuncSetAttribute(chol_diag, cudaFuncAttributeMaxDynamicSharedMemorySize, kBlkSmem));
         CU(cudaFuncSetAttribute(tri_solve_block, cudaFuncAttributeMaxDynamicSharedMemorySize, kBlkSmem));
-        if (cudaMalloc(&plan->chol_info, sizeof(int)) != cudaSuccess) return PTFOCK_ERR_ALLOC;
-        if (cudaMallocHost(&plan->chol_info_host, sizeof(int)) != cudaSuccess) return PTFOCK_ERR_ALLOC;
+        if (!plan->chol_info && cudaMalloc(&plan->chol_info, sizeof(int)) != cudaSuccess) {
+            plan->chol_info = nullptr; cudaGetLastError(); return PTFOCK_ERR_ALLOC;
+        }
+        if (!plan->chol_info_host && cudaMallocHost(&plan->chol_info_host, sizeof(int)) != cudaSuccess) {
+            plan->chol_info_host = nullptr; cudaGetLastError(); return PTFOCK_ERR_ALLOC;
+        }
     }
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     cd *S = plan->scratch, *X = (cd *)psi;
     CU(cudaMemsetAsync(plan->chol_info, 0, sizeof(int), st));
     // S = Psi^* Psi, padded with the identity to a multiple of the block size
@@ -1255,7 +1288,7 @@ extern "C" int ptfock_orthonormalize(ptfock_plan *plan, void *psi, int32_t n, vo
     }
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(plan->chol_info_host, plan->chol_info, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CU(end_call(plan, st));
+    END_CALL();
     CU(cudaStreamSynchronize(st));
     return *plan->chol_info_host ? PTFOCK_ERR_NOT_POSITIVE : PTFOCK_OK;
 }
@@ -1274,20 +1307,42 @@ __global__ void __launch_bounds__(256) add_vloc_kernel(const double *vloc, const
     o.y = fma(v, z.y, o.y);
     out[k] = o;
 }
-// out_j = a_j x_j + b_j y_j (y may be null)
-__global__ void __launch_bounds__(256) axpby_kernel(const cd *coef, int n, const cd *x, const cd *y, cd *out, long long n_pts) {
+// out_j = a_j x_j + b_j y_j (y may be null) for the kAxpbyChunk orbitals from j0 on; the coefficients travel by value in the
+// kernel's parameter space, so the caller's host arrays are free again when the launch returns (pinned or pageable)
+constexpr int kAxpbyChunk = 64;
+struct AxpbyCoef { cd a[kAxpbyChunk], b[kAxpbyChunk]; };
+__global__ void __launch_bounds__(256) axpby_kernel(const __grid_constant__ AxpbyCoef coef, int j0, const cd *x, const cd *y, cd *out, long long n_pts) {
     const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y;
+    const int c = blockIdx.y;
     if (r >= n_pts) return;
-    const long long k = (long long)j * n_pts + r;
-    cd v = cmul(coef[j], x[k]);
-    if (y) v = cadd(v, cmul(coef[n + j], y[k]));
+    const long long k = (long long)(j0 + c) * n_pts + r;
+    cd v = cmul(coef.a[c], x[k]);
+    if (y) v = cadd(v, cmul(coef.b[c], y[k]));
     out[k] = v;
 }
 // part[j][b] = sum over block b's points of conj(a_j) b_j; out[j] = w * sum_b part[j][b] (fixed order)
 __global__ void __launch_bounds__(256) banddot_partial(const cd *a, const cd *b, long long n_pts, int blocks_per, double2 *part) {
     __shared__ double2 red[256];
     const int j = blockIdx.y;
+// v_out = v_ext + g rho (v_ext may be null = 0)
+__global__ void __launch_bounds__(256) vloc_update_kernel(const double *v_ext, double g, const double *rho, double *v_out, long long n_pts) {
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_pts) return;
+    v_out[r] = fma(g, rho[r], v_ext ? v_ext[r] : 0.0);
+}
+// partial[b] = (sum over block b's grid-stride points of |a - b|, 0)
+__global__ void __launch_bounds__(256) absdiff_partial(const double *a, const double *b, long long n, double2 *partial) {
+    __shared__ double red[256];
+    double sacc = 0.0;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) sacc += fabs(a[k] - b[k]);
+    red[threadIdx.x] = sacc;
+    __syncthreads();
+    for (int h = 128; h > 0; h >>= 1) {
+        if (threadIdx.x < h) red[threadIdx.x] += red[threadIdx.x + h];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = make_double2(red[0], 0.0);
+}
     double sr = 0.0, si = 0.0;
     for (long long r = (long long)blockIdx.x * 256 + threadIdx.x; r < n_pts; r += (long long)blocks_per * 256) {
         const cd x = a[(long long)j * n_pts + r], y = b[(long long)j * n_pts + r];
@@ -1315,12 +1370,13 @@ extern "C" int ptfock_hloc_apply(ptfock_plan *plan, const double *vloc, const vo
     if (!plan || !psi || !out || n < 1 || plan->d.kernel != PTFOCK_KERNEL_KINETIC) return PTFOCK_ERR_INVALID_ARG;
     int rc = check_dev_ptrs(plan, { psi, out });
     if (rc != PTFOCK_OK) return rc;
-    if (vloc && ((uintptr_t)vloc & 7)) return PTFOCK_ERR_ALIGNMENT;
+    rc = check_dev_doubles(plan, vloc);
+    if (rc != PTFOCK_OK) return rc;
     const size_t gbytes = sizeof(cd) * (size_t)plan->N;
     if (overlaps(out, gbytes * n, psi, gbytes * n)) return PTFOCK_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     if (!plan->ones) {
         cudaError_t e = cudaMalloc(&plan->ones, gbytes);
         if (e != cudaSuccess) { g_last_cuda = (int)e; return PTFOCK_ERR_ALLOC; }
@@ -1335,7 +1391,7 @@ extern "C" int ptfock_hloc_apply(ptfock_plan *plan, const double *vloc, const vo
         plan->total_launches += 1;
     }
     CU(cudaGetLastError());
-    CU(end_call(plan, st));
+    END_CALL();
     return PTFOCK_OK;
 }
 
@@ -1344,18 +1400,20 @@ extern "C" int ptfock_axpby(ptfock_plan *plan, int32_t n, const double *a_host, 
     if (!plan || !a_host || !x || !out || n < 1 || (y && !b_host)) return PTFOCK_ERR_INVALID_ARG;
     int rc = check_dev_ptrs(plan, { x, y, out });
     if (rc != PTFOCK_OK) return rc;
-    if (sizeof(cd) * 2 * (size_t)n > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
-    // the coefficients travel through the head of the scratch (pageable host memory: the copy is staged by the runtime
-    // before the call returns, so the caller may reuse a_host / b_host at once)
-    CU(cudaMemcpyAsync(plan->scratch, a_host, sizeof(cd) * n, cudaMemcpyHostToDevice, st));
-    if (y) CU(cudaMemcpyAsync(plan->scratch + n, b_host, sizeof(cd) * n, cudaMemcpyHostToDevice, st));
-    axpby_kernel<<<dim3((unsigned)((plan->N + 255) / 256), n), 256, 0, st>>>(plan->scratch, n, (const cd *)x, (const cd *)y, (cd *)out, plan->N);
-    plan->total_launches += 1;
+    BEGIN_CALL(plan, st);
+    for (int j0 = 0; j0 < n; j0 += kAxpbyChunk) {
+        const int nc = std::min(kAxpbyChunk, n - j0);
+        AxpbyCoef coef;
+        std::memset(&coef, 0, sizeof(coef));
+        std::memcpy(coef.a, a_host + 2 * (size_t)j0, sizeof(cd) * nc);
+        if (y) std::memcpy(coef.b, b_host + 2 * (size_t)j0, sizeof(cd) * nc);
+        axpby_kernel<<<dim3((unsigned)((plan->N + 255) / 256), nc), 256, 0, st>>>(coef, j0, (const cd *)x, (const cd *)y, (cd *)out, plan->N);
+        plan->total_launches += 1;
+    }
     CU(cudaGetLastError());
-    CU(end_call(plan, st));
+    END_CALL();
     return PTFOCK_OK;
 }
 
@@ -1367,53 +1425,86 @@ extern "C" int ptfock_banddot(ptfock_plan *plan, const void *a, const void *b, i
     if (sizeof(double2) * (size_t)n * (blocks_per + 1) > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
     cudaStream_t st = (cudaStream_t)stream;
     GUARD(plan->d.device);
-    CU(begin_call(plan, st));
+    BEGIN_CALL(plan, st);
     double2 *part = reinterpret_cast<double2 *>(plan->scratch), *res = part + (size_t)n * blocks_per;
     banddot_partial<<<dim3(blocks_per, n), 256, 0, st>>>((const cd *)a, (const cd *)b, plan->N, blocks_per, part);
     banddot_final<<<(n + 63) / 64, 64, 0, st>>>(part, blocks_per, n, plan->volume / (double)plan->N, res);
     plan->total_launches += 2;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out_host, res, sizeof(double2) * n, cudaMemcpyDeviceToHost, st));
-    CU(end_call(plan, st));
+    END_CALL();
     CU(cudaStreamSynchronize(st));
     return PTFOCK_OK;
 }
 
-namespace {
-int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host);
-}
-extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) { return measure_fp64_peak(device, false, tflops_host); }
-extern "C" int ptfock_measure_dmma_peak(int32_t device, double *tflops_host) { return measure_fp64_peak(device, true, tflops_host); }
-namespace {
-int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host) {
-    if (!tflops_host) return PTFOCK_ERR_INVALID_ARG;
-    GUARD(device);
-    cudaDeviceProp prop;
-    CU(cudaGetDeviceProperties(&prop, device));
-    if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
-    double *sink = nullptr;
-    CU(cudaMalloc(&sink, sizeof(double)));
-    cudaEvent_t e0, e1;
-    CU(cudaEventCreate(&e0));
-    CU(cudaEventCreate(&e1));
-    const int blocks = prop.multiProcessorCount * 8, iters = 1 << 16;
-    double best = 0.0;
-    for (int rep = 0; rep < 6; ++rep) {             // first repetitions warm the clocks up
-        cudaEventRecord(e0, 0);
-        if (tensor) dmma_peak_kernel<<<blocks, 256>>>(sink, iters, 1e-3, 1e-3);
-        else fp64_peak_kernel<<<blocks, 256>>>(sink, iters, 1.0000001, 1e-9);
-        cudaEventRecord(e1, 0);
-        cudaError_t e = cudaEventSynchronize(e1);
-        if (e != cudaSuccess) { g_last_cuda = (int)e; cudaFree(sink); return PTFOCK_ERR_CUDA; }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        // per thread and iteration: 8 DFMAs, or 8 warp-wide 8 x 8 x 4 MMAs (256 FMAs shared by 32 lanes = 8 per lane)
-        const double tf = (tensor ? 8.0 : 1.0) * 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
-        if (rep >= 2 && tf > best) best = tf;
+extern "C" int ptfock_vloc_update(ptfock_plan *plan, const double *v_ext, double g, const double *rho, double *v_out, void *stream) {
+    if (!plan || !rho || !v_out) return PTFOCK_ERR_INVALID_ARG;
+    for (const double *q : { v_ext, rho, (const double *)v_out }) {
+        int rc = check_dev_doubles(plan, q);
+        if (rc != PTFOCK_OK) return rc;
     }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(sink);
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    vloc_update_kernel<<<(unsigned)((plan->N + 255) / 256), 256, 0, st>>>(v_ext, g, rho, v_out, plan->N);
+    plan->total_launches += 1;
+    CU(cudaGetLastError());
+    return PTFOCK_OK;
+}
+
+extern "C" int ptfock_density_change(ptfock_plan *plan, const double *rho_a, const double *rho_b, double *change_host, void *stream) {
+    if (!plan || !rho_a || !rho_b || !change_host) return PTFOCK_ERR_INVALID_ARG;
+    for (const double *q : { rho_a, rho_b }) {
+        int rc = check_dev_doubles(plan, q);
+        if (rc != PTFOCK_OK) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    BEGIN_CALL(plan, st);                                                // plan->partials / result buffers are shared by consecutive calls
+    const int blocks = (int)std::min<long long>(1024, (plan->N + 255) / 256);
+    absdiff_partial<<<blocks, 256, 0, st>>>(rho_a, rho_b, plan->N, plan->partials);
+    dot_final<<<1, 256, 0, st>>>(plan->partials, blocks, plan->volume / (double)plan->N, plan->result_dev);
+    plan->total_launches += 2;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(plan->result_host, plan->result_dev, sizeof(double2), cudaMemcpyDeviceToHost, st));
+    END_CALL();
+    CU(cudaStreamSynchronize(st));
+    *change_host = plan->result_host->x;
+    return PTFOCK_OK;
+}
+
+// out_host[(k * n + j)] = (a_j, b^k_j) for k < n_sets: the inner products of one orbital set with n_sets others in ONE call
+// (one synchronisation): a new row of the Anderson Gram matrices and their right-hand sides
+extern "C" int ptfock_banddot_many(ptfock_plan *plan, const void *a, const void *const *b_sets_host, int32_t n_sets, int32_t n,
+                                   double *out_host, void *stream) {
+    if (!plan || !a || !b_sets_host || !out_host || n < 1 || n_sets < 1) return PTFOCK_ERR_INVALID_ARG;
+    int rc = check_dev_ptrs(plan, { a });
+    if (rc != PTFOCK_OK) return rc;
+    for (int k = 0; k < n_sets; ++k) {
+        if (!b_sets_host[k]) return PTFOCK_ERR_INVALID_ARG;
+        rc = check_dev_ptrs(plan, { b_sets_host[k] });
+        if (rc != PTFOCK_OK) return rc;
+    }
+    const int blocks_per = (int)std::max<long long>(1, std::min<long long>(64, plan->N / 2048));
+    const size_t per_set = (size_t)n * (blocks_per + 1);                 // partial sums + results of one set
+    if (sizeof(double2) * per_set * (size_t)n_sets > plan->scratch_bytes) return PTFOCK_ERR_ALLOC;
+    cudaStream_t st = (cudaStream_t)stream;
+    GUARD(plan->d.device);
+    BEGIN_CALL(plan, st);
+    double2 *part = reinterpret_cast<double2 *>(plan->scratch), *res = part + (size_t)n_sets * n * blocks_per;
+    for (int k = 0; k < n_sets; ++k) {
+        banddot_partial<<<dim3(blocks_per, n), 256, 0, st>>>((const cd *)a, (const cd *)b_sets_host[k], plan->N, blocks_per,
+                                                             part + (size_t)k * n * blocks_per);
+        banddot_final<<<(n + 63) / 64, 64, 0, st>>>(part + (size_t)k * n * blocks_per, blocks_per, n, plan->volume / (double)plan->N,
+                                                     res + (size_t)k * n);
+    }
+    plan->total_launches += 2 * n_sets;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out_host, res, sizeof(double2) * (size_t)n * n_sets, cudaMemcpyDeviceToHost, st));
+    END_CALL();
+    CU(cudaStreamSynchronize(st));
+    return PTFOCK_OK;
+}
+
 // ---- ptfock_banddot_static: the same two kernels with their partial sums in a built-in array (no allocation) ----------
 // For callers that must not trigger a cudaMalloc (all HBM owned by their own pool, or a loop whose other streams a
 // device-wide synchronising allocation would stall); see include/ptfock.h.
@@ -1472,6 +1563,41 @@ extern "C" int ptfock_banddot_static(int32_t device, int64_t n_points, double we
     return PTFOCK_OK;
 }
 }  // namespace
+namespace {
+int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host);
+}
+extern "C" int ptfock_measure_dfma_peak(int32_t device, double *tflops_host) { return measure_fp64_peak(device, false, tflops_host); }
+extern "C" int ptfock_measure_dmma_peak(int32_t device, double *tflops_host) { return measure_fp64_peak(device, true, tflops_host); }
+namespace {
+int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host) {
+    if (!tflops_host) return PTFOCK_ERR_INVALID_ARG;
+    GUARD(device);
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return PTFOCK_ERR_UNSUPPORTED_DEVICE;
+    double *sink = nullptr;
+    CU(cudaMalloc(&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 8, iters = 1 << 16;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {             // first repetitions warm the clocks up
+        cudaEventRecord(e0, 0);
+        if (tensor) dmma_peak_kernel<<<blocks, 256>>>(sink, iters, 1e-3, 1e-3);
+        else fp64_peak_kernel<<<blocks, 256>>>(sink, iters, 1.0000001, 1e-9);
+        cudaEventRecord(e1, 0);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; cudaFree(sink); return PTFOCK_ERR_CUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        // per thread and iteration: 8 DFMAs, or 8 warp-wide 8 x 8 x 4 MMAs (256 FMAs shared by 32 lanes = 8 per lane)
+        const double tf = (tensor ? 8.0 : 1.0) * 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+        if (rep >= 2 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
 
 extern "C" int ptfock_measure_copy_bandwidth(int32_t device, uint64_t bytes, int32_t reps, double *gbs_host) {
     if (!gbs_host || bytes < 4096 || reps < 1) return PTFOCK_ERR_INVALID_ARG;

@@ -5,8 +5,8 @@
 
 A real Hamiltonian needs the pseudopotentials the paper uses, which are not available; the model keeps
 the structure of the step.  This module only SEQUENCES library calls: every operation on grids runs in the kernels of
-libptfock.so (ptfock_apply, ptfock_hloc_apply, ptfock_residual, ptfock_density, ptfock_axpby, ptfock_banddot,
-ptfock_orthonormalize); the host solves the (<= 20 x 20) per-wavefunction least-squares problems of the Anderson
+libptfock.so (ptfock_apply, ptfock_hloc_apply, ptfock_residual, ptfock_density, ptfock_vloc_update, ptfock_density_change,
+ptfock_axpby, ptfock_banddot, ptfock_banddot_many, ptfock_orthonormalize); the host solves the (<= 20 x 20) per-wavefunction least-squares problems of the Anderson
 mixing, as the paper's "size of the least squares problem becomes very small".  No CPU fallback.
 """
 from __future__ import annotations
@@ -42,7 +42,7 @@ class PTCN:
         """H[Psi] Psi (Alg. 1 line 5: the potential and the exchange operator follow Psi_f)."""
         v = self.v_ext
         if self.g != 0.0:
-            v = torch_add_scaled(self.v_ext, self.fock.density(psi), self.g)
+            v = self.fock.vloc_update(self.v_ext, self.g, self.fock.density(psi))
         out = self.kin.hloc_apply(psi, v)
         if self.alpha != 0.0:
             vx = self.fock.apply(psi)                                   # Psi = Phi: pair-symmetric schedule
@@ -72,7 +72,7 @@ class PTCN:
             if x_prev is not None:
                 dxs.insert(0, f.axpby(1.0, psi_f, -1.0, x_prev))
                 drs.insert(0, f.axpby(1.0, r_f, -1.0, r_prev))
-                row = np.stack([f.banddot(drs[0], d) for d in drs], axis=1)        # <dR_new, dR_b> for every stored b
+                row = f.banddot_many(drs[0], drs).T                     # <dR_new, dR_b> for every stored b, one call
                 m_old = gram.shape[1]
                 g2 = np.empty((n_e, m_old + 1, m_old + 1), dtype=np.complex128)
                 g2[:, 1:, 1:] = gram
@@ -88,7 +88,7 @@ class PTCN:
             m = len(dxs)
             new = f.axpby(1.0, psi_f, -beta, r_f)                       # line 7: Anderson mixing, per wavefunction
             if m > 0:
-                rhs = np.stack([f.banddot(d, r_f) for d in drs], axis=1)
+                rhs = f.banddot_many(r_f, drs).conj().T                 # <dR_b, R_f> = conj <R_f, dR_b>, one call
                 gamma = np.empty((n_e, m), dtype=np.complex128)
                 for j in range(n_e):
                     gj = gram[j] + 1e-14 * np.trace(gram[j]).real / m * np.eye(m)
@@ -98,14 +98,11 @@ class PTCN:
                     f.axpby(1.0, new, beta * gamma[:, a], drs[a], out=new)
             psi_f = new
             rho_new = f.density(psi_f)                                  # line 8
-            change = float((rho_new - rho).abs().sum()) * self.w / n_e  # a reduction of the monitor, not of the method
+            change = f.density_change(rho_new, rho) / n_e               # line 9
             rho = rho_new
             info.update(iterations=it + 1, rho_change=change)
+        info["psi_f"] = psi_f                                           # the fixed point of Eq. (5) before line 11
         out = psi_f.clone()
         f.orthonormalize(out)                                           # line 11
         return out, info
 
-
-def torch_add_scaled(a, b, s):
-    """a + s b for two real grids (the local potential v_ext + g rho; input plumbing of the model, not the method)."""
-    return (a + s * b).contiguous()

@@ -48,6 +48,25 @@ def test_overlap_rotate_density_small(cuda_device, n, na, nb):
     assert _rel(rho.cpu().numpy(), oracle.density(an)) <= TOL
 
 
+@pytest.mark.parametrize("n_orb", [1, 64, 70, 200])
+def test_hermitian_overlap_computes_the_lower_tiles_and_mirrors_the_rest(cuda_device, n_orb):
+    """S = Psi^* Psi: with the same orbitals on both sides only the 64 x 64 tiles on and below the diagonal
+    are contracted; the others are their conjugate mirror images.  Against the oracle, and against the general path."""
+    n = (16, 16, 32)
+    cfg = synth.Config("h", (9.0, 10.0, 11.0), n, n_orb, synth.KERNEL_HSE)
+    a = _noise((n_orb,) + n, 31, cuda_device)
+    w = cfg.volume / cfg.N
+    with binding.plan_for(cfg) as plan:
+        herm = plan.overlap(a, a).cpu().numpy()                         # same pointer: Hermitian path
+        full = plan.overlap(a, a.clone()).cpu().numpy()                 # another pointer: every tile contracted
+    assert _rel(herm, oracle.overlap(a.cpu().numpy(), a.cpu().numpy(), w)) <= TOL
+    assert np.array_equal(herm, herm.conj().T) or _rel(herm, herm.conj().T) <= 1e-15
+    t = np.arange(n_orb) // 64
+    low = t[:, None] >= t[None, :]
+    assert np.array_equal(herm[low], full[low])                         # computed tiles: the same sums
+    assert _rel(herm, full) <= 1e-14
+
+
 @pytest.mark.parametrize("n_orb", [1, 5, 64, 70, 130])
 def test_residuals_and_orthonormalize_small(cuda_device, n_orb):
     n = (16, 16, 16)
@@ -106,6 +125,21 @@ def test_Si512_sizes_sampled(cuda_device):
         # R_n is orthogonal to the (orthonormal) Psi: Psi^* R_n = 0 at any size
         z = plan.overlap(psi, rn)
         assert float(z.abs().max()) <= 1e-11 * float(s.abs().max())
+        # R_n and R_f element by element on sampled orbitals (both sides of a 64-wide tile edge, first and last), from the
+        # oracle's overlap and rotation over ALL 1024 orbitals (Alg. 3 lines 2, 4, 5; a full
+        # oracle.residual would take hours): R_n[c] = H psi_c - sum_m psi_m S[m][c], S[:, c] = (psi_m, H psi_c)
+        cols, dt = [0, 63, 64, 1023], 0.37
+        half = _noise(tuple(psi.shape), 10, cuda_device)
+        rf = plan.residual(psi, hpsi, dt=dt, psi_half=half)
+        torch.cuda.synchronize()
+        psi_np = psi.cpu().numpy()
+        h_c = np.ascontiguousarray(hpsi[cols].cpu().numpy())
+        proj = oracle.rotate(psi_np, oracle.overlap(psi_np, h_c, w))
+        ref_rn = h_c - proj
+        ref_rf = psi_np[cols] + 0.5j * dt * ref_rn - half[cols].cpu().numpy()
+        assert np.abs(rn[cols].cpu().numpy() - ref_rn).max() <= TOL * np.abs(ref_rn).max()
+        assert np.abs(rf[cols].cpu().numpy() - ref_rf).max() <= TOL * np.abs(ref_rf).max()
+        del psi_np, rf, half
         # density: sampled points against the oracle's definition, and the electron count
         pts = [0, 12345, 262143]
         flat = psi.reshape(1024, -1)
@@ -132,6 +166,7 @@ def test_Si1536_orbital_count_sampled(cuda_device):
     w = cfg.volume / cfg.N
     with binding.plan_for(cfg) as plan:
         keep = psi[[0, 1, 70, 3071]].clone()
+        head = psi[:70].cpu().numpy()                                   # columns 0..69 of Psi L^-H depend on these only
         s = plan.overlap(psi, psi)
         plan.orthonormalize(psi)
         s2 = plan.overlap(psi, psi)
@@ -146,3 +181,7 @@ def test_Si1536_orbital_count_sampled(cuda_device):
     assert np.abs(psi[1].cpu().numpy().ravel() - q1).max() <= 1e-12 * np.abs(q1).max()
     ref = w * np.vdot(keep[2].cpu().numpy().ravel(), keep[3].cpu().numpy().ravel())
     assert abs(s[70, 3071].item() - ref) <= TOL * float(s.abs().max())
+    # the first 70 columns (across the first 64-wide Cholesky panel) against the oracle: L is lower triangular, so column k of
+    # Psi L^-H is fixed by orbitals 0..k and oracle.orthonormalize of the leading 70 orbitals gives exactly these columns
+    ref_head = oracle.orthonormalize(np.ascontiguousarray(head), w)
+    assert np.abs(psi[:70].cpu().numpy() - ref_head).max() <= 1e-11 * np.abs(ref_head).max()

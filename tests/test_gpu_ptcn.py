@@ -45,6 +45,46 @@ def test_step_helpers(cuda_device):
         d = st.fock.banddot(psi, y)
         ref_d = np.array([st.w * np.vdot(psi[j].cpu().numpy().ravel(), y[j].cpu().numpy().ravel()) for j in range(5)])
         assert np.abs(d - ref_d).max() <= 1e-13
+        # one call for several sets: same kernels, same order of summation as ptfock_banddot, set by set
+        z_t = torch.from_numpy(z).to(cuda_device)
+        many = st.fock.banddot_many(psi, [y, z_t, psi])
+        assert many.shape == (3, 5)
+        for k, other in enumerate([y, z_t, psi]):
+            assert np.array_equal(many[k], st.fock.banddot(psi, other))
+        # Alg. 1 line 5 (potential follows the density) and line 9 (density change), against their definitions
+        rho = st.fock.density(psi)
+        rho2 = st.fock.density(y + 0.1 * z_t)
+        vl = st.fock.vloc_update(st.v_ext, 0.5, rho).cpu().numpy()
+        assert np.abs(vl - (v + 0.5 * rho.cpu().numpy())).max() <= 1e-15 * np.abs(vl).max() * 2
+        assert np.array_equal(st.fock.vloc_update(None, 2.0, rho).cpu().numpy(), 2.0 * rho.cpu().numpy())
+        ch = st.fock.density_change(rho, rho2)
+        ref_ch = st.w * np.abs(rho.cpu().numpy() - rho2.cpu().numpy()).sum()
+        assert ref_ch > 1e-3 and abs(ch - ref_ch) <= 1e-13 * ref_ch
+        assert st.fock.density_change(rho, rho) == 0.0
+
+
+def test_axpby_many_orbitals_pinned_coefficients_reused_at_once(cuda_device):
+    """70 orbitals = two launches of 64 + 6 coefficient sets passed by value; the PINNED host arrays are overwritten right
+    after the call returns (ptfock.h: "may be reused when the call returns") and must not change the result."""
+    cfg = synth.Config("axp", (9.0, 10.0, 11.0), (16, 16, 16), 70, synth.KERNEL_HSE)
+    x = synth.random_orbitals(cfg, 41, 70, cuda_device)
+    y = synth.random_orbitals(cfg, 42, 70, cuda_device)
+    rng = np.random.default_rng(5)
+    a = rng.standard_normal(70) + 1j * rng.standard_normal(70)
+    b = rng.standard_normal(70) + 1j * rng.standard_normal(70)
+    ah, bh = torch.from_numpy(a.copy()).pin_memory(), torch.from_numpy(b.copy()).pin_memory()
+    out = torch.empty_like(x)
+    with binding.plan_for(cfg) as plan:
+        rc = binding.lib().ptfock_axpby(plan._h, 70, ah.data_ptr(), x.data_ptr(), bh.data_ptr(), y.data_ptr(), out.data_ptr(),
+                                        torch.cuda.current_stream().cuda_stream)
+        ah.zero_()
+        bh.zero_()
+        assert rc == 0
+        torch.cuda.synchronize()
+        only_a = plan.axpby(a, x).cpu().numpy()
+    ref = a[:, None, None, None] * x.cpu().numpy() + b[:, None, None, None] * y.cpu().numpy()
+    assert np.abs(out.cpu().numpy() - ref).max() <= 4e-15 * np.abs(ref).max()
+    assert np.abs(only_a - a[:, None, None, None] * x.cpu().numpy()).max() <= 4e-15 * np.abs(ref).max()
 
 
 @pytest.mark.parametrize("alpha,g", [(0.0, 0.0), (0.25, 0.5)], ids=["linear", "exchange+density"])
@@ -63,6 +103,32 @@ def test_one_step_matches_oracle(cuda_device, alpha, g):
     rho, rho_ref = (np.abs(got) ** 2).sum(0), (np.abs(ref) ** 2).sum(0)
     assert np.abs(rho - rho_ref).max() <= 1e-9 * rho_ref.max()
     assert np.abs(got - psi0.cpu().numpy()).max() > 1e-3 * np.abs(ref).max()        # the step did move the orbitals
+
+
+def test_step_at_32cube_with_70_orbitals_is_the_fixed_point_the_oracle_defines(cuda_device):
+    """A step at a size that reaches the real kernels: 32^3 two-stage slab / pencil passes, the pair-symmetric schedule,
+    a 64-wide tile edge in the tensor-core overlap / rotation and in the blocked Cholesky (70 = 64 + 6 orbitals), two
+    coefficient chunks in ptfock_axpby.  The oracle's own iteration needs minutes here (its route to the fixed point is
+    22 exchange applications), so it judges the RESULT instead: Eq. (5) has one solution near Psi_{n+1/2}, and the GPU's
+    un-orthogonalised Psi_f must satisfy it under the oracle's operators (Alg. 1 lines 1, 2, 5, 6 evaluated by
+    oracle.ptcn_ref / oracle.residual), and line 11 must equal oracle.orthonormalize of that Psi_f."""
+    n, edges, n_e, dt = (32, 32, 32), (9.0, 10.0, 11.0), 70, 0.05
+    cell, v, psi0, ref_model = _model(n, edges, n_e, 0.25, 0.5, cuda_device)
+    with ptcn.PTCN(cell, n, n_e, alpha=0.25, v_ext=torch.from_numpy(v), g=0.5) as st:
+        out, info = st.step(psi0, dt, tol=1e-11, max_iter=80)
+        torch.cuda.synchronize()
+        finfo = st.fock.info()
+    assert finfo["pass8"] == 1 and finfo["last_symmetric"] == 1          # two-stage kernels, i <= j schedule
+    assert info["residual"] < 1e-11 and info["iterations"] < 80
+    p0, pf, w = psi0.cpu().numpy(), info["psi_f"].cpu().numpy(), ref_model.w
+    r_n = oracle.residual(p0, ref_model.h_apply(p0), w)                                             # line 1
+    psi_half = np.ascontiguousarray(p0 - 0.5j * dt * r_n)                                           # line 2
+    r_f = oracle.residual(pf, ref_model.h_apply(pf), w, dt=dt, psi_half=psi_half)                   # lines 5-6
+    per_band = np.sqrt(w * (np.abs(r_f) ** 2).reshape(n_e, -1).sum(1))
+    assert per_band.max() <= 1e-10, per_band.max()
+    assert np.abs(pf - psi_half).max() > 1e-4 * np.abs(pf).max()         # the iteration did move away from its start
+    ref_out = oracle.orthonormalize(pf, w)                                                          # line 11
+    assert np.abs(out.cpu().numpy() - ref_out).max() <= 1e-10 * np.abs(ref_out).max()
 
 
 def test_sharded_apply_world1_equals_apply(cuda_device):

@@ -55,4 +55,6 @@ def test_workspace_bound_keeps_one_slot(cuda_device):
     with binding.plan_for(cfg, block_i=2, block_j=2, workspace_bytes=4 * pair) as one, \
             binding.plan_for(cfg, block_i=2, block_j=2, workspace_bytes=8 * pair) as two:
         assert one.info()["slots"] == 1 and two.info()["slots"] == 2
+        # the bound is an upper bound on the whole scratch: the dense-algebra minimum does not inflate it (ptfock.h)
+        assert one.info()["scratch_bytes"] <= 4 * pair and two.info()["scratch_bytes"] <= 8 * pair
         assert torch.equal(one.apply(phi, psi), two.apply(phi, psi))
