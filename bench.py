@@ -257,8 +257,14 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
                 "executed_pair_solves_per_s": rate,      # `value` is the EFFECTIVE rate n_i * n_j / time
                 "bytes_model": "72 N per executed pair-solve (SURVEY.md 8(d) B_3pass); own model below",
                 "own_bytes_per_pair_solve": sum(per_pair), "own_bytes_frac": rate / (peak * 1e9 / sum(per_pair)),
+                "frac_note": "frac uses the 72 N contract model on the timed region's rate; this build moves own_bytes_per_pair_solve "
+                             "(< 72 N), so own_bytes_frac is the fraction of the peak its own traffic reaches",
                 "worst_pass_frac": min(v["frac"] for v in per_kernel.values()),
-                "dominant_kernel": names[k], "per_kernel": per_kernel, "traffic": None}
+                "dominant_kernel": names[k], "per_kernel": per_kernel,
+                "per_kernel_schedule": "separate profiling step after the timed region: single stream, every launch bracketed by "
+                                       "CUDA events on the launching stream (the timed region itself runs two waves on two "
+                                       "streams with no per-launch events)",
+                "traffic": None, "traffic_source": None}
     try:
         import math
         p64 = binding.measure_fp64_peak(local)
@@ -271,6 +277,9 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             roofline["traffic"] = json.load(f).get(cfg.name, {}).get(names[k].split(" ")[0])
+        if roofline["traffic"] is not None:
+            roofline["traffic_source"] = ("profiles/traffic.json: dram bytes per launch from an ncu --set full capture of an "
+                                          "earlier run of the same kernel, not measured in this run")
     except Exception:
         pass
 
@@ -333,7 +342,7 @@ def measure(cfg, args, dev, local, rank, world, steps, warmup, do_e2e, do_cpu, c
             "vs_baseline": (value / world / PAPER_PAIRS_PER_S[cfg.name]) if cfg.name in PAPER_PAIRS_PER_S else None}
 
 
-def dense_leg(cfg, args, dev, local):
+def dense_leg(cfg, args, dev, local, emit=True):
     """--leg dense: the dense-algebra neighbours (Alg. 3, Sec. 3.4) at cfg's sizes, each
     timed alone with CUDA events on the launching stream; roofline = the plain FP64 pipe (measured live) for the
     contractions, HBM for the density."""
@@ -376,7 +385,9 @@ def dense_leg(cfg, args, dev, local):
                                                 16.0 * N * n * n, 80.0 * N * n),
             "density (Sec. 3.4)": (lambda: plan.density(psi, out=rho), None, 4.0 * N * n, 16.0 * N * n),
             "orthonormalize (Sec. 3.4: overlap + Cholesky + Trsm)": (lambda: plan.orthonormalize(work), lambda: work.copy_(mix),
-                                                                    12.0 * N * n * n + 4.0 / 3.0 * n ** 3, 48.0 * N * n),
+                                                                    # Hermitian overlap on the lower tiles (4 N n^2 of the full
+                                                                    # 8 N n^2) + triangular solve (4 N n^2) + Cholesky
+                                                                    8.0 * N * n * n + 4.0 / 3.0 * n ** 3, 48.0 * N * n),
         }
         for name, (fn, setup, flops, byts) in legs.items():
             ms = timed(fn, args.steps, setup)
@@ -390,10 +401,12 @@ def dense_leg(cfg, args, dev, local):
             "roofline": {"tensor_peak_tflops": p64, "tensor_peak_source": "measured live (ptfock_measure_dmma_peak: fp64 mma.sync m8n8k4)",
                          "fma_peak_tflops": p64_fma,
                          "hbm_peak_gbs": peak_hbm, "per_call": out}}
-    print(json.dumps(line), flush=True)
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
-def ptcn_leg(cfg, args, dev, local):
+def ptcn_leg(cfg, args, dev, local, emit=True):
     """--leg ptcn: whole PT-CN time steps (Algorithm 1: residual, Anderson-mixed fixed point, density,
     re-orthogonalisation) with the model Hamiltonian of DESIGN.md Q17 at cfg's grid and orbital count, sequenced over
     the C ABI by paper_1905_01348_b200/ptcn.py; wall time per step (host least-squares included) and the share of it
@@ -438,7 +451,82 @@ def ptcn_leg(cfg, args, dev, local):
             "dtype": "f64", "data": "synthetic", "steps": args.steps, "higher_is_better": False,
             "fock_exchange_share": statistics.median(s["fock_exchange_ms"] / s["ms"] for s in steps_out),
             "per_step": steps_out}
-    print(json.dumps(line), flush=True)
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
+
+
+def cufft_leg(cfg, args, dev, local, emit=True, n_targets=None):
+    """--leg cufft: SIDE COMPARISON only (north_star: "cuFFT-based runs may be timed only as a side comparison").  The paper's
+    own method on this GPU (Sec. 3.2 items 1-2: batched cuFFT with custom kernels in the gaps), written
+    with torch: batched torch.fft.fftn / ifftn (cuFFT) and element-wise torch ops for the pair product, the v(G) multiply,
+    the phi_i multiply and the sum over i.  Nothing of this is linked into libptfock.so or used by the product path.
+    Times a slice (all orbitals x n_targets targets) with CUDA events and compares the result with ptfock_apply."""
+    import numpy as np
+    import torch
+    from paper_1905_01348_b200 import binding, synth
+    n_i = cfg.n_occ
+    n_j = n_targets or (cfg.j_block if cfg.j_block else min(cfg.n_occ, 64))
+    phi = synth.orbitals(cfg, cfg.seed_phi, n_i, dev)
+    psi = synth.orbitals(cfg, cfg.seed_psi, n_j, dev) if cfg.separate_psi else phi[:n_j].clone()
+    # v(G) on torch's FFT frequency order; m_d in [-n_d/2, n_d/2), G = m B, B = 2 pi inv(A)^T (include/ptfock.h)
+    a = np.asarray(cfg.cell, dtype=np.float64).reshape(3, 3)
+    b = 2.0 * np.pi * np.linalg.inv(a).T
+    ms = [np.where(np.arange(k) < (k + 1) // 2, np.arange(k), np.arange(k) - k) for k in cfg.n]
+    m0, m1, m2 = np.meshgrid(*ms, indexing="ij")
+    g = m0[..., None] * b[0] + m1[..., None] * b[1] + m2[..., None] * b[2]
+    g2 = (g * g).sum(-1)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        if cfg.kernel == 1:
+            v = np.where(g2 > 0, 4 * np.pi / g2 * -np.expm1(-g2 / (4 * cfg.omega ** 2)), np.pi / cfg.omega ** 2)
+        else:
+            v = np.where(g2 > 0, 4 * np.pi / g2, 0.0)
+    v_t = torch.from_numpy(-cfg.alpha * v).to(dev)
+    N = cfg.N
+    # batch: as many pair densities per cuFFT call as ~4 GB allow (input, output and cuFFT's workspace live together)
+    ib = max(1, min(n_i, int((4 << 30) // (16 * N))))
+    out = torch.zeros((n_j,) + tuple(cfg.n), dtype=torch.complex128, device=dev)
+
+    def run():
+        out.zero_()
+        for j in range(n_j):
+            for i0 in range(0, n_i, ib):
+                p = phi[i0:i0 + ib]
+                w = torch.fft.fftn(p.conj() * psi[j], dim=(-3, -2, -1))
+                w *= v_t
+                w = torch.fft.ifftn(w, dim=(-3, -2, -1))
+                out[j] += (p * w).sum(0)
+    run()                                                                # warm-up (plans, allocator)
+    torch.cuda.synchronize()
+    reps = max(1, min(3, args.steps))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        run()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_run = e0.elapsed_time(e1) / reps
+    with binding.plan_for(cfg, device=local, max_targets=n_j) as plan:
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ours = plan.apply(phi, psi)
+        t0.record()
+        for _ in range(reps):
+            plan.apply(phi, psi, out=ours)
+        t1.record()
+        torch.cuda.synchronize()
+        ms_ours = t0.elapsed_time(t1) / reps
+    diff = float((ours - out).abs().max() / ours.abs().max())
+    pairs = n_i * n_j
+    line = {"metric": "cuFFT side comparison: batched torch.fft + element-wise torch ops (the paper's method, PAPER.md:148-149)",
+            "side_comparison": True, "unit": UNIT, "value": pairs / (ms_run * 1e-3), "ptfock_value_same_slice": pairs / (ms_ours * 1e-3),
+            "ptfock_over_cufft": ms_run / ms_ours, "max_rel_diff_vs_ptfock": diff, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {n_j} targets x {n_i} orbitals (general schedule on both sides)", "leg": "cufft",
+                       "grid": list(cfg.n), "pairs_per_cufft_batch": ib, "reps": reps}}
+    del phi, psi, out
+    torch.cuda.empty_cache()
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
 def main():
@@ -461,7 +549,7 @@ def main():
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the second headline config (one Si1536 j-block) that the default Si512 run also times")
     ap.add_argument("--check", action="store_true", help="also compare sampled output columns with the oracle")
-    ap.add_argument("--leg", default="fock", choices=["fock", "dense", "copybw", "ptcn"],
+    ap.add_argument("--leg", default="fock", choices=["fock", "dense", "copybw", "ptcn", "cufft"],
                     help="fock: the headline exchange path (default); dense: the dense-algebra neighbours; copybw: device "
                          "copy bandwidth vs working-set size (L2-resident vs HBM; profiles/r02_l2_resident.md); ptcn: whole PT-CN time "
                          "steps with the model Hamiltonian (use --config Si64 / Si216); own JSON lines")
@@ -499,9 +587,9 @@ def main():
         if dist is not None:
             dist.destroy_process_group()
         return
-    if args.leg in ("dense", "ptcn"):
+    if args.leg in ("dense", "ptcn", "cufft"):
         if rank == 0:
-            (dense_leg if args.leg == "dense" else ptcn_leg)(cfg, args, dev, local)
+            {"dense": dense_leg, "ptcn": ptcn_leg, "cufft": cufft_leg}[args.leg](cfg, args, dev, local)
         if dist is not None:
             dist.destroy_process_group()
         return
@@ -514,6 +602,20 @@ def main():
             second = measure(synth.CONFIGS["Si1536"], args, dev, local, rank, world, 3, 2, False, False)
         except Exception as e:                      # e.g. not enough free memory: the headline line still prints
             second = {"error": f"{type(e).__name__}: {e}"}
+
+    # bounded extras of the default run (a few seconds each, after the timed region): the dense-algebra neighbours at the
+    # headline size, one PT-CN step at Si64, and the cuFFT side comparison on a 32-target slice
+    extras = {}
+    if rank == 0 and cfg.name == "Si512" and not args.no_secondary and not args.targets and world == 1:
+        small = argparse.Namespace(**dict(vars(args), steps=2))
+        for name, fn in (("dense", lambda: dense_leg(cfg, small, dev, local, emit=False)),
+                         ("ptcn", lambda: ptcn_leg(synth.CONFIGS["Si64"], small, dev, local, emit=False)),
+                         ("cufft", lambda: cufft_leg(cfg, small, dev, local, emit=False, n_targets=32))):
+            try:
+                extras[name] = fn()
+            except Exception as e:                  # never lose the headline line to an extra
+                extras[name] = {"error": f"{type(e).__name__}: {e}"}
+            torch.cuda.empty_cache()
 
     if rank == 0:
         line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -535,6 +637,11 @@ def main():
                 line["survey_72N_frac_Si1536"] = second["roofline"]["survey_72N_frac"]
         if m["parity"]:
             line["parity"] = m["parity"]
+        if extras:
+            line["config"]["secondary_legs"] = {k: v for k, v in extras.items() if k != "cufft"}
+            if "cufft" in extras:
+                line["side_comparison_cufft"] = extras["cufft"]
+                line["vs_cufft"] = extras["cufft"].get("ptfock_over_cufft")
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

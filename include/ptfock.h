@@ -28,8 +28,11 @@
  *
  * Supported grids: n0 in {16, 32, 48, 64, 120, 128}; (n1, n2) one of the built slab shapes
  *   (64,64) (128,48) (48,48) (32,32) (90,60)            -- TMA-fed three-stage slab passes
- *   (16,16) (16,32) (32,16) (16,48) (48,32) (32,64)     -- generic slab passes
- * (all BASELINE.json configs, and the paper's own 60 x 90 x 120 grid stored as 120 x 90 x 60).
+ *   every other pair from {16, 32, 48, 64, 128}^2 except (128,128)   -- generic slab passes
+ * (all BASELINE.json configs, the paper's own 60 x 90 x 120 grid stored as 120 x 90 x 60, and 120 of the 125 grids with
+ * edges from {16, 32, 48, 64, 128}; a 128 x 128 slab, 256 KB of complex fp64, does not fit one CTA's shared memory and
+ * has no kernel yet: n0 x 128 x 128 returns PTFOCK_ERR_UNSUPPORTED_GRID -- store such a cell with a shorter axis last
+ * two, e.g. 128 x 128 x 64 instead of 64 x 128 x 128).
  * 64 x 64 x 64, 48 x 48 x 48 and 32 x 32 x 32 additionally have the two-stage slab passes + two-stage pencil pass, and 16 x 16 x 16
  * the single-pass on-chip kernel (whole pair-solve in one CTA, no scratch); these are the default for their grids.
  * The dense-algebra contractions (ptfock_overlap / rotate / residual / orthonormalize) run on the FP64 tensor cores.
@@ -234,13 +237,13 @@ int ptfock_density_change(ptfock_plan *plan, const double *rho_a, const double *
 int ptfock_banddot_static(int32_t device, int64_t n_points, double weight, const void *a, const void *b, int32_t n,
                           void *out, void *stream);
 
-const char *ptfock_strerror(int code);
-
-/* The cudaError_t of the most recent PTFOCK_ERR_CUDA on this thread (0 if none). */
 /* Frees everything the plan owns.  NULL is allowed. */
 int ptfock_destroy(ptfock_plan *plan);
 
 /* Static string for an error code. */
+const char *ptfock_strerror(int code);
+
+/* The cudaError_t of the most recent PTFOCK_ERR_CUDA on this thread (0 if none). */
 int ptfock_last_cuda_error(void);
 
 /* Introspection for the harness (host memory, no device work):

@@ -105,6 +105,10 @@ typedef SX<90, 60, 6, 15, 4, 15, true, false> SX_90x60;        // paper grid 120
 const SlabEntry kSlabs[] = {
     SLABX(SX_64x64), SLABX(SX_128x48), SLABX(SX_48x48), SLABX(SX_32x32), SLABX(SX_90x60),
     SLAB(16, 16), SLAB(16, 32), SLAB(32, 16), SLAB(16, 48), SLAB(48, 32), SLAB(32, 64),
+    // the rest of {16, 32, 48, 64, 128}^2 (north_star (1): "grid edges 16/32/48/64/128") on the generic passes; only the
+    // 128 x 128 slab is missing: 256 KB of complex fp64 do not fit one CTA's shared memory
+    SLAB(16, 64), SLAB(16, 128), SLAB(32, 48), SLAB(32, 128), SLAB(48, 16), SLAB(48, 64), SLAB(48, 128),
+    SLAB(64, 16), SLAB(64, 32), SLAB(64, 48), SLAB(64, 128), SLAB(128, 16), SLAB(128, 32), SLAB(128, 64),
 };
 #undef SLAB
 #undef SLABX
@@ -593,17 +597,17 @@ extern "C" const char *ptfock_strerror(int code) {
     switch (code) {
         case PTFOCK_OK: return "ok";
         case PTFOCK_ERR_INVALID_ARG: return "invalid argument";
-        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (n0 in {16,32,48,64,120,128}; (n1,n2) one of the built slab shapes, see ptfock.h)";
+        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (n0 in {16,32,48,64,120,128}; (n1,n2) from {16,32,48,64,128}^2 except (128,128), or (90,60); see ptfock.h)";
         case PTFOCK_ERR_UNSUPPORTED_DEVICE: return "unsupported device (needs compute capability 10.x; there is no CPU fallback)";
         case PTFOCK_ERR_ALIGNMENT: return "pointer not 16-byte aligned";
         case PTFOCK_ERR_ALLOC: return "allocation failed or workspace too small";
         case PTFOCK_ERR_CUDA: return "CUDA runtime error (see ptfock_last_cuda_error)";
         case PTFOCK_ERR_ALIAS: return "out overlaps an input";
         case PTFOCK_ERR_NOT_POSITIVE: return "overlap matrix is not positive definite (linearly dependent orbitals)";
+        case PTFOCK_ERR_TOO_LARGE: return "too many bands for the built-in scratch (ptfock_banddot_static: n <= PTFOCK_STATIC_MAX_BANDS = 4096; split the call)";
         default: return "unknown error";
     }
 }
-        case PTFOCK_ERR_TOO_LARGE: return "too many bands for the built-in scratch (ptfock_banddot_static: n <= PTFOCK_STATIC_MAX_BANDS = 4096; split the call)";
 
 extern "C" int ptfock_last_cuda_error(void) { return g_last_cuda; }
 
@@ -650,10 +654,6 @@ cudaError_t end_call(ptfock_plan *p, cudaStream_t st) {
     if (e == cudaSuccess) { p->last_stream = st; p->has_last = 1; }
     return e;
 }
-
-// profiling: record an event that closes an interval of kind `tag` (-1: opens a new run of intervals)
-void mark(Wave &w, int tag) {
-    ptfock_plan *p = w.p;
 // an error return after begin_call may already have queued work on `st` (a first-use fill, part of a wave): the busy
 // event is recorded on EVERY way out, so that the next call on another stream is still ordered behind it
 struct CallScope {
@@ -665,6 +665,10 @@ struct CallScope {
 };
 #define BEGIN_CALL(plan_, st_) CU(begin_call(plan_, st_)); CallScope call_scope__{ plan_, st_, false }
 #define END_CALL() CU(call_scope__.close())
+
+// profiling: record an event that closes an interval of kind `tag` (-1: opens a new run of intervals)
+void mark(Wave &w, int tag) {
+    ptfock_plan *p = w.p;
     if (!p->profiling) return;
     if (!p->ev_pool) { p->ev_pool = new std::vector<cudaEvent_t>(); p->ev_tags = new std::vector<int>(); }
     if (p->ev_used == p->ev_pool->size()) {
@@ -1320,10 +1324,6 @@ __global__ void __launch_bounds__(256) axpby_kernel(const __grid_constant__ Axpb
     if (y) v = cadd(v, cmul(coef.b[c], y[k]));
     out[k] = v;
 }
-// part[j][b] = sum over block b's points of conj(a_j) b_j; out[j] = w * sum_b part[j][b] (fixed order)
-__global__ void __launch_bounds__(256) banddot_partial(const cd *a, const cd *b, long long n_pts, int blocks_per, double2 *part) {
-    __shared__ double2 red[256];
-    const int j = blockIdx.y;
 // v_out = v_ext + g rho (v_ext may be null = 0)
 __global__ void __launch_bounds__(256) vloc_update_kernel(const double *v_ext, double g, const double *rho, double *v_out, long long n_pts) {
     const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1343,6 +1343,10 @@ __global__ void __launch_bounds__(256) absdiff_partial(const double *a, const do
     }
     if (threadIdx.x == 0) partial[blockIdx.x] = make_double2(red[0], 0.0);
 }
+// part[j][b] = sum over block b's points of conj(a_j) b_j; out[j] = w * sum_b part[j][b] (fixed order)
+__global__ void __launch_bounds__(256) banddot_partial(const cd *a, const cd *b, long long n_pts, int blocks_per, double2 *part) {
+    __shared__ double2 red[256];
+    const int j = blockIdx.y;
     double sr = 0.0, si = 0.0;
     for (long long r = (long long)blockIdx.x * 256 + threadIdx.x; r < n_pts; r += (long long)blocks_per * 256) {
         const cd x = a[(long long)j * n_pts + r], y = b[(long long)j * n_pts + r];
@@ -1559,10 +1563,6 @@ extern "C" int ptfock_banddot_static(int32_t device, int64_t n_points, double we
     return PTFOCK_OK;
 }
 
-    *tflops_host = best;
-    return PTFOCK_OK;
-}
-}  // namespace
 namespace {
 int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host);
 }
@@ -1598,6 +1598,10 @@ int measure_fp64_peak(int32_t device, bool tensor, double *tflops_host) {
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(sink);
+    *tflops_host = best;
+    return PTFOCK_OK;
+}
+}  // namespace
 
 extern "C" int ptfock_measure_copy_bandwidth(int32_t device, uint64_t bytes, int32_t reps, double *gbs_host) {
     if (!gbs_host || bytes < 4096 || reps < 1) return PTFOCK_ERR_INVALID_ARG;

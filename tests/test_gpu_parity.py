@@ -51,6 +51,27 @@ def test_small_grids_every_codelet(cuda_device, case):
     assert _rel(out.cpu().numpy(), _oracle(cfg, phi, psi)) <= TOL
 
 
+# every slab shape (n1, n2) from {16, 32, 48, 64, 128}^2 that round 3 opened on the generic passes (north_star (1): "grid
+# edges 16/32/48/64/128"; include/ptfock.h), on a 16-point pencil axis, plus three of them under long pencils
+OPENED = [(16, n1, n2) for n1, n2 in [(16, 64), (16, 128), (32, 48), (32, 128), (48, 16), (48, 64), (48, 128), (64, 16), (64, 32),
+                                      (64, 48), (64, 128), (128, 16), (128, 32), (128, 64)]] + \
+         [(64, 64, 128), (128, 128, 64), (48, 64, 48)]
+
+
+@pytest.mark.parametrize("n", OPENED, ids=["x".join(map(str, n)) for n in OPENED])
+def test_opened_slab_shapes(cuda_device, n):
+    edges = tuple(0.64 * k + 0.1 * d for d, k in enumerate(n))          # anisotropic spacing: a swapped axis shows
+    cfg = synth.Config("open", edges, n, 2, synth.KERNEL_HSE, separate_psi=True)
+    phi = synth.random_orbitals(cfg, 71, 2, cuda_device)
+    psi = synth.random_orbitals(cfg, 72, 2, cuda_device)
+    with binding.plan_for(cfg, max_targets=2) as plan:
+        out = plan.apply(phi, psi)
+        sym = plan.apply(phi)                                           # Psi = Phi: the pair-symmetric schedule
+        torch.cuda.synchronize()
+    assert _rel(out.cpu().numpy(), _oracle(cfg, phi, psi)) <= TOL
+    assert _rel(sym.cpu().numpy(), _oracle(cfg, phi)) <= TOL
+
+
 def test_debug_pair_matches_oracle_W(cuda_device):
     cfg = synth.Config("w", (9.0, 17.0, 12.0), (16, 32, 16), 2, synth.KERNEL_HSE, alpha=0.25)
     ab = synth.random_orbitals(cfg, 5, 2, cuda_device)
