@@ -597,7 +597,7 @@ extern "C" const char *ptfock_strerror(int code) {
     switch (code) {
         case PTFOCK_OK: return "ok";
         case PTFOCK_ERR_INVALID_ARG: return "invalid argument";
-        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (n0 in {16,32,48,64,120,128}; (n1,n2) from {16,32,48,64,128}^2 except (128,128), or (90,60); see ptfock.h)";
+        case PTFOCK_ERR_UNSUPPORTED_GRID: return "unsupported grid (n0 in {16,32,48,64,120,128}; built slab shapes (n1,n2): {16,32,48,64,128}^2 except (128,128), and (90,60); see ptfock.h)";
         case PTFOCK_ERR_UNSUPPORTED_DEVICE: return "unsupported device (needs compute capability 10.x; there is no CPU fallback)";
         case PTFOCK_ERR_ALIGNMENT: return "pointer not 16-byte aligned";
         case PTFOCK_ERR_ALLOC: return "allocation failed or workspace too small";
